@@ -1,0 +1,149 @@
+/*
+ * triples_b200.h -- C ABI of the B200 (sm_100a) closed-shell CCSD(T) perturbative triples energy.
+ *
+ * What it computes (arXiv:1609.08094, section 2.2):
+ *
+ *   Eq. (2.2.2), L94 : t_ijk^abc eps_ijk^abc = -P_ijk^abc [ sum_d t_ij^ad g_ckbd - sum_l t_il^ab g_cklj ]
+ *   Eq. (2.2.3), L99 : P x_ijk^abc = x_ijk^abc + x_ikj^acb + x_jik^bac + x_jki^bca + x_kij^cab + x_kji^cba
+ *   Eq. (2.2.4): z_ijk^abc eps_ijk^abc = -( t_i^a g_jbkc + t_j^b g_iakc + t_k^c g_iajb )
+ *   Eq. (2.2.5): x~^abc = 2 ( 2/3 x^abc - x^acb + 1/3 x^bca )
+ *   Eq. (2.2.1), L87 : E[4] = sum t~ t eps,  E[5] = sum z~ t eps,  E(T) = E[4] + E[5]
+ *
+ * evaluated over the restricted occupied triplets i<=j<=k (L119; task count Eq. (5.0.7b))
+ * with the readings of DESIGN.md ("Readings"): D = eps_i+eps_j+eps_k-eps_a-eps_b-eps_c (< 0),
+ *   W^abc  = numerator of Eq. (2.2.2) after P,   Vd^abc = numerator of Eq. (2.2.4),
+ *   e_ijk  = sum_abc Z[W]^abc (W + Vd)^abc / D^abc,
+ *   Z[W]^abc = 4W^abc + W^bca + W^cab - 2W^acb - 2W^cba - 2W^bac,
+ *   E(T)   = sum_{i<=j<=k} (2 - delta_ij - delta_jk) e_ijk           (so E(T) < 0).
+ *
+ * Conventions for every entry point
+ *   - Tensors are dense, row-major (C order), last index fastest, float64, no padding.
+ *     Mulliken integrals (L63): vvvo[a][b][c][k] = (ab|ck), ovoo[i][a][j][k] = (ia|jk),
+ *     ovov[i][a][j][b] = (ia|jb); t1[i][a] = t_i^a; t2[i][j][a][b] = t_ij^ab.
+ *     Preconditions (not checked on the hot path): real orbitals (8-fold integral symmetry),
+ *     t2[i][j][a][b] == t2[j][i][b][a], every D != 0.
+ *   - "device" pointers are CUDA device pointers on the current device, 16-byte aligned;
+ *     "host" pointers are ordinary host memory.  All pointers are caller-owned; inputs are
+ *     never modified or freed.  The library allocates no device memory: all scratch comes from
+ *     `workspace` (device, caller-owned, e.g. a torch.uint8 tensor), 256-byte aligned.
+ *   - Work is enqueued on `cuda_stream` (a cudaStream_t, may be NULL for the default stream);
+ *     the call synchronises that stream once before writing host outputs.
+ *   - Errors: a triples_status_t is returned, nothing aborts or throws; a message for the last
+ *     non-OK status of the calling thread is available from triples_last_error().
+ *     There is no CPU fallback: on a device that is not compute capability 10.x the compute
+ *     entry points return TRIPLES_EARCH.
+ *   - precision: TRIPLES_FP64  = contractions in FP64 (DMMA), everything FP64;
+ *                TRIPLES_MIXED = the paper's mixed precision (L125, L156): only the W build
+ *                (the contractions) in single precision (3xTF32 split on tcgen05, FP32
+ *                accumulate, W stored FP32); Vd, D, the energy reduction and sums in FP64.
+ */
+#ifndef TRIPLES_B200_H
+#define TRIPLES_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { TRIPLES_FP64 = 0, TRIPLES_MIXED = 1 } triples_precision_t;
+
+typedef enum {
+    TRIPLES_OK = 0,
+    TRIPLES_EINVAL = 1,      /* bad size, null or misaligned pointer, unknown precision, bad triplet */
+    TRIPLES_EWORKSPACE = 2,  /* workspace too small: re-query triples_workspace_bytes */
+    TRIPLES_ECUDA = 3,       /* a CUDA call failed; text in triples_last_error() */
+    TRIPLES_EARCH = 4        /* device is not compute capability 10.x */
+} triples_status_t;
+
+/* Number of restricted triplets T = nocc(nocc+1)(nocc+2)/6 (Eq. (5.0.7b)); 0 if nocc < 1. */
+long long triples_triplet_count(int nocc);
+
+/* Enumeration order of the restricted loop: for i in [0,o): for j in [i,o): for k in [j,o).
+ * ijk_out: host, 3*T ints.  This is the index order of e_triplet_out below. */
+int triples_triplet_list(int nocc, int* ijk_out);
+
+/* Bytes of device workspace triples_energy needs for (nocc, nvirt, precision); 0 on invalid
+ * arguments.  Host-only computation, no CUDA call. */
+size_t triples_workspace_bytes(int nocc, int nvirt, int precision);
+
+/* Same for triples_energy_host (adds room for device copies of the seven inputs). */
+size_t triples_workspace_bytes_host(int nocc, int nvirt, int precision);
+
+/*
+ * E(T) of Eq. (2.2.1)-(2.2.5) with all inputs resident on the device.
+ *   eps_o[nocc], eps_v[nvirt], t1, t2, vvvo, ovoo, ovov : device, float64 (layouts above)
+ *   e_out          : host, 3 doubles: e_out[0] = E(T), e_out[1] = E[4], e_out[2] = E[5]
+ *   e_triplet_out  : device, 3*T doubles or NULL: for triplet n of triples_triplet_list,
+ *                    [3n+0] = w*(e4+e5), [3n+1] = w*e4, [3n+2] = w*e5, w = 2-d_ij-d_jk
+ * All sums are taken in a fixed order (no atomics): results are run-to-run bitwise identical.
+ */
+int triples_energy(int nocc, int nvirt,
+                   const double* eps_o, const double* eps_v, const double* t1, const double* t2,
+                   const double* vvvo, const double* ovoo, const double* ovov,
+                   int precision,
+                   void* workspace, size_t workspace_bytes, void* cuda_stream,
+                   double* e_out, double* e_triplet_out);
+
+/*
+ * Same computation with all seven inputs in HOST memory (pinned or pageable): the library copies
+ * them into `workspace` (device) on `cuda_stream`, runs triples_energy, and copies the results
+ * back.  e_out: host, 3 doubles; e_triplet_out: HOST, 3*T doubles or NULL.
+ */
+int triples_energy_host(int nocc, int nvirt,
+                        const double* eps_o, const double* eps_v, const double* t1, const double* t2,
+                        const double* vvvo, const double* ovoo, const double* ovov,
+                        int precision,
+                        void* workspace, size_t workspace_bytes, void* cuda_stream,
+                        double* e_out, double* e_triplet_out);
+
+/*
+ * Per-triplet energies of a caller-chosen list of restricted triplets (the sampled-parity
+ * protocol for the configurations whose full oracle run is out of reach).
+ *   ntrip, ijk (host, 3*ntrip ints, each 0 <= i <= j <= k < nocc)
+ *   e_out: host, 3*ntrip doubles, layout as e_triplet_out above (weighted).
+ * Workspace requirement: triples_workspace_bytes.
+ */
+int triples_energy_subset(int nocc, int nvirt,
+                          const double* eps_o, const double* eps_v, const double* t1, const double* t2,
+                          const double* vvvo, const double* ovoo, const double* ovov,
+                          int precision, int ntrip, const int* ijk,
+                          void* workspace, size_t workspace_bytes, void* cuda_stream,
+                          double* e_out);
+
+/*
+ * W_ijk^abc = P_ijk^abc [ sum_d t_ij^ad g_ckbd - sum_l t_il^ab g_cklj ]  (Eq. (2.2.2)-(2.2.3))
+ * for ONE ordered (i,j,k), any order, written as float64 W_out[a][b][c] (device, nvirt^3 doubles).
+ * Runs the same contraction kernels as triples_energy (in `precision`) followed by the
+ * permutation-accumulate; meant for elementwise parity tests of the contraction stage.
+ */
+int triples_w_block(int nocc, int nvirt,
+                    const double* t2, const double* vvvo, const double* ovoo,
+                    int precision, int i, int j, int k,
+                    void* workspace, size_t workspace_bytes, void* cuda_stream,
+                    double* W_out);
+
+/*
+ * Timing of the calling thread's last triples_energy / _host / _subset call, measured with CUDA
+ * events on `cuda_stream` when profiling was switched on with triples_set_profiling(1) before it.
+ *   out[0] prepare (repack) ms          out[1] contraction kernels, summed ms
+ *   out[2] contraction launches         out[3] fused reduction kernels, summed ms
+ *   out[4] reduction launches           out[5] other kernels (finalize/sum), summed ms
+ *   out[6] other launches               out[7] contraction flops executed (12v^4+12ov^3 per
+ *                                              triplet, coinciding terms of i=j / j=k computed once)
+ *   out[8] reduction algorithmic bytes  out[9] triplets executed (i=j=k skipped)
+ * Returns TRIPLES_EINVAL if no profiled call has happened.
+ */
+int triples_last_profile(double* out10);
+void triples_set_profiling(int on);
+
+/* Thread-local message for the last non-OK status ("" if none). Never NULL. */
+const char* triples_last_error(void);
+
+/* ABI version of this header (integer, bumped on any signature change). */
+int triples_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TRIPLES_B200_H */

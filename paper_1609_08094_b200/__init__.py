@@ -1,0 +1,21 @@
+"""B200 (sm_100a) closed-shell CCSD(T) perturbative triples energy, arXiv:1609.08094 section 2.2.
+
+The product is the C-ABI library of ``include/triples_b200.h`` (CUDA kernels in ``csrc/``); this package is
+its thin Python binding (``binding``) plus the seeded synthetic-input generator (``synth``) shared by the
+tests and the benchmark.  There is no CPU fallback: the binding raises if the CUDA library is missing.
+"""
+from .binding import (  # noqa: F401
+    FP64,
+    MIXED,
+    TriplesError,
+    triples_energy,
+    triples_energy_host,
+    triples_energy_subset,
+    triples_last_profile,
+    triples_set_profiling,
+    triples_triplet_count,
+    triples_triplet_list,
+    triples_w_block,
+    triples_workspace_bytes,
+    triples_workspace_bytes_host,
+)

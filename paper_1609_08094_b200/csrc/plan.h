@@ -1,0 +1,141 @@
+// plan.h -- host-side planner (S1 of DESIGN.md): triplet enumeration, tile-orbit table, batching, workspace layout.
+// Pure host arithmetic (no CUDA calls) so that the CPU test-suite can exercise it through the C ABI.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <vector>
+
+namespace tb {
+
+constexpr int kMaxVirt = 2040;   // tile indices of the 8-wide reduction tiles fit a byte
+constexpr int kMaxOcc = 1024;
+constexpr int kNumSM = 148;
+
+struct Triplet { int i, j, k; long long index; };   // index = position in the i<=j<=k enumeration
+
+inline long long triplet_count(int o) { return o < 1 ? 0 : (long long)o * (o + 1) * (o + 2) / 6; }
+
+// Enumeration order of the restricted loop (count Eq. (5.0.7b)).
+inline void enumerate_triplets(int o, std::vector<Triplet>& out) {
+    out.clear();
+    long long n = 0;
+    for (int i = 0; i < o; ++i)
+        for (int j = i; j < o; ++j)
+            for (int k = j; k < o; ++k) out.push_back({i, j, k, n++});
+}
+
+// Position of (i<=j<=k) in that enumeration, closed form.
+inline long long triplet_index(int o, int i, int j, int k) {
+    // triplets with first index < i: sum_{x<i} (o-x)(o-x+1)/2 = T(o) - T(o-i)
+    auto T3 = [](long long n) { return n * (n + 1) * (n + 2) / 6; };
+    auto T2 = [](long long n) { return n * (n + 1) / 2; };
+    const long long m = o - i;                     // j,k range over [i,o): m values
+    return T3(o) - T3(m) + (T2(m) - T2(m - (j - i))) + (k - j);
+}
+
+// Weight of a restricted triplet (Q4): 2 - delta_ij - delta_jk.
+inline double triplet_weight(int i, int j, int k) { return 2.0 - (i == j ? 1.0 : 0.0) - (j == k ? 1.0 : 0.0); }
+
+struct Orbit { uint8_t A, B, C, sym; };   // tiles A<=B<=C of the virtual cube; sym = |stabiliser| in {1,2,6}
+
+inline int num_red_tiles(int v) { return (v + 7) / 8; }
+inline long long orbit_count(int v) { const long long n = num_red_tiles(v); return n * (n + 1) * (n + 2) / 6; }
+inline void enumerate_orbits(int v, std::vector<Orbit>& out) {
+    out.clear();
+    const int n = num_red_tiles(v);
+    for (int A = 0; A < n; ++A)
+        for (int B = A; B < n; ++B)
+            for (int C = B; C < n; ++C) {
+                const int sym = (A == B && B == C) ? 6 : ((A == B || B == C) ? 2 : 1);
+                out.push_back({(uint8_t)A, (uint8_t)B, (uint8_t)C, (uint8_t)sym});
+            }
+}
+
+enum GemmCfgId { CFG_M120_N128 = 0, CFG_M80_N192 = 1, CFG_M40_N256 = 2 };
+
+struct Plan {
+    int o = 0, v = 0, vp = 0, op = 0, prec = 0;
+    int cfg = 0, BM = 0, BN = 0, mtiles = 0, ntiles = 0;
+    int nb = 0;                 // triplets per batch
+    long long T = 0;            // restricted triplets
+    int norb = 0;
+    size_t esz = 8;             // bytes per stored operand / U element
+    size_t n_x = 0, n_ot = 0, n_t2 = 0, n_u = 0;   // elements of one X (or XT), Ot, T2, one U buffer
+    // workspace offsets (bytes)
+    size_t off_x = 0, off_xt = 0, off_ot = 0, off_t2 = 0, off_xlo = 0, off_xtlo = 0, off_otlo = 0, off_t2lo = 0;
+    size_t off_u = 0, off_part = 0, off_etrip = 0, off_result = 0, off_gjobs = 0, off_rjobs = 0, off_fjobs = 0,
+           off_orb = 0;
+    size_t total = 0;
+    // host variant: device copies of the inputs follow
+    size_t off_in[7] = {0, 0, 0, 0, 0, 0, 0};
+    size_t in_bytes[7] = {0, 0, 0, 0, 0, 0, 0};
+    size_t total_host = 0;
+};
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Returns false on invalid sizes.  precision: 0 = FP64, 1 = MIXED.
+inline bool make_plan(int o, int v, int prec, Plan& P) {
+    if (o < 1 || v < 1 || o > kMaxOcc || v > kMaxVirt || (prec != 0 && prec != 1)) return false;
+    P = Plan();
+    P.o = o; P.v = v; P.prec = prec;
+    P.vp = (v + 1) & ~1;
+    P.op = (o + 1) & ~1;
+    P.esz = prec == 0 ? 8 : 4;
+    P.T = triplet_count(o);
+    P.norb = (int)orbit_count(v);
+    // CTA tile: the M tile (40, 80 or 120 rows) that wastes the fewest padded rows; ties -> larger tile
+    const int bms[3] = {120, 80, 40};
+    const int ids[3] = {CFG_M120_N128, CFG_M80_N192, CFG_M40_N256};
+    const int bns[3] = {128, 192, 256};
+    long long best = -1;
+    for (int c = 0; c < 3; ++c) {
+        const long long padded = (long long)((v + bms[c] - 1) / bms[c]) * bms[c];
+        if (best < 0 || padded < best) { best = padded; P.cfg = ids[c]; P.BM = bms[c]; P.BN = bns[c]; }
+    }
+    const long long N = (long long)v * P.vp;
+    P.mtiles = (v + P.BM - 1) / P.BM;
+    P.ntiles = (int)((N + P.BN - 1) / P.BN);
+    P.n_x = (size_t)o * v * v * P.vp;
+    P.n_ot = (size_t)o * o * v * P.op;
+    P.n_t2 = (size_t)o * o * v * P.vp;
+    P.n_u = (size_t)v * v * P.vp;
+    // batch: enough CTAs for >= 40 waves of 148 SMs, U buffers capped at 12 GiB, at least one triplet
+    const long long ctas_per_triplet = 3LL * P.mtiles * P.ntiles;
+    long long nb = (40LL * kNumSM + ctas_per_triplet - 1) / ctas_per_triplet;
+    const long long cap = (long long)((12ULL << 30) / (3 * P.n_u * P.esz));
+    if (nb > cap) nb = cap;
+    if (nb > P.T) nb = P.T;
+    if (nb > 20000) nb = 20000;   // gridDim.y limit of the contraction launch (3 jobs per triplet)
+    if (nb < 1) nb = 1;
+    P.nb = (int)nb;
+
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t at = off; off = align_up(off + bytes, 1024); return at; };
+    P.off_x = take(P.n_x * P.esz);
+    P.off_xt = take(P.n_x * P.esz);
+    P.off_ot = take(P.n_ot * P.esz);
+    P.off_t2 = take(P.n_t2 * P.esz);
+    if (prec == 1) {   // low parts of the hi/lo split
+        P.off_xlo = take(P.n_x * P.esz);
+        P.off_xtlo = take(P.n_x * P.esz);
+        P.off_otlo = take(P.n_ot * P.esz);
+        P.off_t2lo = take(P.n_t2 * P.esz);
+    }
+    P.off_u = take((size_t)P.nb * 3 * P.n_u * P.esz);
+    P.off_part = take((size_t)P.nb * P.norb * 16);
+    P.off_etrip = take((size_t)P.T * 3 * 8);
+    P.off_result = take(256);
+    P.off_gjobs = take((size_t)P.T * 3 * 32);
+    P.off_rjobs = take((size_t)P.T * 48);
+    P.off_fjobs = take((size_t)P.T * 16);
+    P.off_orb = take((size_t)P.norb * 4);
+    P.total = off;
+    const size_t in_elems[7] = {(size_t)o, (size_t)v, (size_t)o * v, (size_t)o * o * v * v, (size_t)v * v * v * o,
+                                (size_t)o * v * o * o, (size_t)o * v * o * v};
+    for (int n = 0; n < 7; ++n) { P.in_bytes[n] = in_elems[n] * 8; P.off_in[n] = take(P.in_bytes[n]); }
+    P.total_host = off;
+    return true;
+}
+
+}  // namespace tb

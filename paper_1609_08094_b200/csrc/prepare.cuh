@@ -1,0 +1,99 @@
+// prepare.cuh -- one-time operand repack (S0 of DESIGN.md; the paper's analogue is the host->device tile
+// transfer).  All outputs live in the caller's workspace.
+//   X [r][d][b][c] = vvvo[d][b][c][r] = (db|cr)        (c-pitch vp = v rounded up to even, pad zeroed)
+//   XT[r][d][b][c] = X[r][d][c][b]
+//   Ot[r][p][a][l] = -ovoo[p][a][l][r] = -(pa|lr)      (l-pitch op = o rounded up to even, pad zeroed)
+//   T2[p][q][a][d] = t2[p][q][a][d]                    (d-pitch vp, pad zeroed)
+// TO is the operand type of the contraction path (double, or float for the mixed path's hi/lo split).
+#pragma once
+#include <cstdint>
+
+namespace tb {
+
+// hi/lo split of a double into two floats: hi = RN_tf32-representable part, lo = remainder (also tf32-rounded).
+// Used only by the mixed path; see gemm_tf32.cuh.
+__device__ __forceinline__ float to_tf32_rn(float x) {
+    uint32_t u;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(x));
+    return __uint_as_float(u);
+}
+
+template <typename TO> struct Splitter;
+template <> struct Splitter<double> {
+    static __device__ __forceinline__ void put(double* hi, double*, size_t idx, double x) { hi[idx] = x; }
+};
+template <> struct Splitter<float> {
+    static __device__ __forceinline__ void put(float* hi, float* lo, size_t idx, double x) {
+        const float h = to_tf32_rn((float)x);
+        hi[idx] = h;
+        if (lo) lo[idx] = to_tf32_rn((float)(x - (double)h));
+    }
+};
+
+// vvvo viewed as [R = v^3][o]: each CTA moves RB consecutive rows (one contiguous span) through smem.
+template <typename TO>
+__global__ void __launch_bounds__(256)
+pack_x_kernel(const double* __restrict__ vvvo, int v, int vp, int o, int RB, TO* __restrict__ X, TO* __restrict__ Xlo) {
+    extern __shared__ double tile[];   // [RB][o+1]
+    const size_t R = (size_t)v * v * v;
+    const size_t R0 = (size_t)blockIdx.x * RB;
+    const int rows = (int)min((size_t)RB, R - R0);
+    const int op1 = o + 1;
+    for (int e = threadIdx.x; e < rows * o; e += 256) {
+        const int rr = e / o, k = e % o;
+        tile[rr * op1 + k] = vvvo[R0 * o + e];
+    }
+    __syncthreads();
+    const size_t plane = (size_t)v * v * vp;   // one r-slice of X
+    for (int e = threadIdx.x; e < rows * o; e += 256) {
+        const int k = e / rows, rr = e % rows;
+        const size_t Rg = R0 + rr;
+        const size_t db = Rg / v;
+        const int c = (int)(Rg % v);
+        Splitter<TO>::put(X, Xlo, (size_t)k * plane + db * vp + c, tile[rr * op1 + k]);
+    }
+}
+
+// XT[r][d][b][c] = X[r][d][c][b]: tile transpose of every (r,d) plane.  blockIdx.z = r*v + d.
+template <typename TO>
+__global__ void __launch_bounds__(256)
+transpose_planes_kernel(const TO* __restrict__ X, int v, int vp, TO* __restrict__ XT) {
+    __shared__ TO tile[32][33];
+    const size_t base = (size_t)blockIdx.z * v * vp;
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int yy = ty; yy < 32; yy += 8)
+        if (y0 + yy < v && x0 + tx < v) tile[yy][tx] = X[base + (size_t)(y0 + yy) * vp + x0 + tx];
+    __syncthreads();
+    for (int yy = ty; yy < 32; yy += 8)
+        if (x0 + yy < v && y0 + tx < v) XT[base + (size_t)(x0 + yy) * vp + y0 + tx] = tile[tx][yy];
+}
+
+// Ot[r][p][a][l] = -ovoo[p][a][l][r]
+template <typename TO>
+__global__ void pack_ot_kernel(const double* __restrict__ ovoo, int v, int o, int op, TO* __restrict__ Ot,
+                               TO* __restrict__ Otlo) {
+    const size_t n = (size_t)o * o * v * o;
+    for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const int l = (int)(e % o);
+        const int a = (int)((e / o) % v);
+        const int p = (int)((e / ((size_t)o * v)) % o);
+        const int r = (int)(e / ((size_t)o * v * o));
+        const double x = -ovoo[(((size_t)p * v + a) * o + l) * o + r];
+        Splitter<TO>::put(Ot, Otlo, (((size_t)r * o + p) * v + a) * op + l, x);
+    }
+}
+
+// T2[p][q][a][d] (d-pitch vp) = t2[p][q][a][d]
+template <typename TO>
+__global__ void pack_t2_kernel(const double* __restrict__ t2, size_t rows, int v, int vp, TO* __restrict__ T2,
+                               TO* __restrict__ T2lo) {
+    const size_t n = rows * v;
+    for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const size_t row = e / v;
+        const int d = (int)(e % v);
+        Splitter<TO>::put(T2, T2lo, row * vp + d, t2[e]);
+    }
+}
+
+}  // namespace tb

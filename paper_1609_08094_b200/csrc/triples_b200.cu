@@ -1,0 +1,509 @@
+// triples_b200.cu -- C-ABI entry points of include/triples_b200.h and the host-side driver.
+// No CPU fallback: every step of the hot path runs in the kernels of gemm_f64.cuh / gemm_tf32.cuh / reduce.cuh.
+#include "../../include/triples_b200.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "gemm_f64.cuh"
+#include "plan.h"
+#include "prepare.cuh"
+#include "reduce.cuh"
+
+namespace {
+
+using namespace tb;
+
+thread_local std::string g_err;
+thread_local double g_prof[10];
+thread_local bool g_prof_valid = false;
+thread_local int g_profiling = 0;
+
+int fail(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+
+#define CU_TRY(expr)                                                                                  \
+    do {                                                                                              \
+        cudaError_t _e = (expr);                                                                      \
+        if (_e != cudaSuccess)                                                                        \
+            return fail(TRIPLES_ECUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+    } while (0)
+
+// ------------------------------------------------------------------------------------------ tensor maps
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int get_encode_fn(EncodeTiledFn* fn) {
+    static EncodeTiledFn cached = nullptr;
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lk(mu);
+    if (!cached) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        CU_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres));
+        if (qres != cudaDriverEntryPointSuccess || !p) return fail(TRIPLES_ECUDA, "cuTensorMapEncodeTiled unavailable");
+        cached = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    *fn = cached;
+    return TRIPLES_OK;
+}
+
+// 3-D map over a dense tensor: dims d0 (fastest) .. d2, strides in elements for d1, d2; 128-byte swizzle.
+int make_map3(CUtensorMap* m, CUtensorMapDataType dt, size_t esz, const void* base, uint64_t d0, uint64_t d1,
+              uint64_t d2, uint64_t s1, uint64_t s2, uint32_t b0, uint32_t b1, uint32_t b2) {
+    EncodeTiledFn fn;
+    if (int rc = get_encode_fn(&fn)) return rc;
+    cuuint64_t dims[3] = {d0, d1, d2};
+    cuuint64_t strides[2] = {s1 * esz, s2 * esz};
+    cuuint32_t box[3] = {b0, b1, b2};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = fn(m, dt, 3, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS)
+        return fail(TRIPLES_ECUDA, "cuTensorMapEncodeTiled failed (%d) dims=%llu,%llu,%llu box=%u,%u,%u", (int)r,
+                    (unsigned long long)d0, (unsigned long long)d1, (unsigned long long)d2, b0, b1, b2);
+    return TRIPLES_OK;
+}
+
+// ------------------------------------------------------------------------------------------ device checks
+int check_device() {
+    int dev = 0;
+    CU_TRY(cudaGetDevice(&dev));
+    int major = 0;
+    CU_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return fail(TRIPLES_EARCH, "device %d has compute capability %d.x; this library is sm_100a only", dev, major);
+    return TRIPLES_OK;
+}
+
+bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) != 0; }
+
+// ------------------------------------------------------------------------------------------ event pool
+struct EventPool {
+    std::vector<cudaEvent_t> ev;
+    size_t used = 0;
+    int get(cudaEvent_t* e) {
+        if (used == ev.size()) {
+            cudaEvent_t n;
+            CU_TRY(cudaEventCreate(&n));
+            ev.push_back(n);
+        }
+        *e = ev[used++];
+        return TRIPLES_OK;
+    }
+    void reset() { used = 0; }
+};
+thread_local EventPool g_events;
+
+// ------------------------------------------------------------------------------------------ contraction launch
+template <int WM, int WN, int NT, int STAGES>
+int launch_gemm_f64(const GemmMaps& maps, const GemmJob* jobs, int njobs, const Plan& P, cudaStream_t st) {
+    using C = GemmF64Cfg<WM, WN, NT, STAGES>;
+    auto kern = gemm_f64_kernel<WM, WN, NT, STAGES>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        attr_set = true;
+    }
+    dim3 grid(P.mtiles * P.ntiles, njobs);
+    kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(maps, jobs, P.v, P.vp, P.o, P.mtiles);
+    CU_TRY(cudaGetLastError());
+    return TRIPLES_OK;
+}
+
+struct Operands {   // device pointers of the repacked operands (workspace) for one precision
+    void *x, *xt, *ot, *t2;
+    void *xlo, *xtlo, *otlo, *t2lo;
+};
+
+int build_maps_f64(const Plan& P, const Operands& op, GemmMaps* maps) {
+    const uint64_t o = P.o, v = P.v, vp = P.vp, opp = P.op, N = v * vp;
+    const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
+    int rc;
+    if ((rc = make_map3(&maps->t2a, dt, 8, op.t2, v, v, o * o, vp, v * vp, 16, P.BM, 1))) return rc;
+    if ((rc = make_map3(&maps->ota, dt, 8, op.ot, o, v, o * o, opp, v * opp, 16, P.BM, 1))) return rc;
+    if ((rc = make_map3(&maps->x, dt, 8, op.x, N, v, o, N, v * N, 16, 16, 1))) return rc;
+    if ((rc = make_map3(&maps->xt, dt, 8, op.xt, N, v, o, N, v * N, 16, 16, 1))) return rc;
+    if ((rc = make_map3(&maps->t2bq, dt, 8, op.t2, N, o, o, N, o * N, 16, 16, 1))) return rc;
+    if ((rc = make_map3(&maps->t2br, dt, 8, op.t2, N, o, o, N, o * N, 16, 1, 16))) return rc;
+    return TRIPLES_OK;
+}
+
+int launch_gemm(const Plan& P, const GemmMaps& maps, const GemmJob* jobs, int njobs, cudaStream_t st) {
+    if (P.prec != TRIPLES_FP64) return fail(TRIPLES_EINVAL, "mixed-precision contraction path is not built in this version");
+    switch (P.cfg) {
+        case CFG_M120_N128: return launch_gemm_f64<3, 4, 4, 4>(maps, jobs, njobs, P, st);
+        case CFG_M80_N192: return launch_gemm_f64<2, 4, 6, 4>(maps, jobs, njobs, P, st);
+        default: return launch_gemm_f64<1, 8, 4, 4>(maps, jobs, njobs, P, st);
+    }
+}
+
+// ------------------------------------------------------------------------------------------ prepare (S0)
+template <typename TO>
+int run_prepare(const Plan& P, const double* t2, const double* vvvo, const double* ovoo, const Operands& op,
+                cudaStream_t st) {
+    const int o = P.o, v = P.v;
+    const bool split = P.prec == TRIPLES_MIXED;
+    if (P.vp != v) {   // zero the pad columns
+        CU_TRY(cudaMemsetAsync(op.x, 0, P.n_x * sizeof(TO), st));
+        CU_TRY(cudaMemsetAsync(op.t2, 0, P.n_t2 * sizeof(TO), st));
+        if (split) {
+            CU_TRY(cudaMemsetAsync(op.xlo, 0, P.n_x * sizeof(TO), st));
+            CU_TRY(cudaMemsetAsync(op.t2lo, 0, P.n_t2 * sizeof(TO), st));
+        }
+    }
+    // XT pads: rows b of a plane have vp entries, entry c = v is never written by the transpose
+    if (P.vp != v) {
+        CU_TRY(cudaMemsetAsync(op.xt, 0, P.n_x * sizeof(TO), st));
+        if (split) CU_TRY(cudaMemsetAsync(op.xtlo, 0, P.n_x * sizeof(TO), st));
+    }
+    if (P.op != o) {
+        CU_TRY(cudaMemsetAsync(op.ot, 0, P.n_ot * sizeof(TO), st));
+        if (split) CU_TRY(cudaMemsetAsync(op.otlo, 0, P.n_ot * sizeof(TO), st));
+    }
+    {   // X
+        int RB = 128;
+        while ((size_t)RB * (o + 1) * 8 > 64 * 1024 && RB > 1) RB /= 2;
+        const size_t R = (size_t)v * v * v;
+        const size_t smem = (size_t)RB * (o + 1) * 8;
+        auto kern = pack_x_kernel<TO>;
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
+        kern<<<(unsigned)((R + RB - 1) / RB), 256, smem, st>>>(vvvo, v, P.vp, o, RB, (TO*)op.x, (TO*)op.xlo);
+        CU_TRY(cudaGetLastError());
+    }
+    {   // XT (and its low part)
+        dim3 grid((v + 31) / 32, (v + 31) / 32, 1);
+        // gridDim.z <= 65535: loop over r-slices
+        for (int r = 0; r < o; ++r) {
+            grid.z = v;
+            const size_t sl = (size_t)r * v * v * P.vp;
+            transpose_planes_kernel<TO><<<grid, 256, 0, st>>>((const TO*)op.x + sl, v, P.vp, (TO*)op.xt + sl);
+            if (split)
+                transpose_planes_kernel<TO><<<grid, 256, 0, st>>>((const TO*)op.xlo + sl, v, P.vp, (TO*)op.xtlo + sl);
+        }
+        CU_TRY(cudaGetLastError());
+    }
+    pack_ot_kernel<TO><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.op, (TO*)op.ot, (TO*)op.otlo);
+    CU_TRY(cudaGetLastError());
+    pack_t2_kernel<TO><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vp, (TO*)op.t2, (TO*)op.t2lo);
+    CU_TRY(cudaGetLastError());
+    return TRIPLES_OK;
+}
+
+Operands carve_operands(const Plan& P, uint8_t* ws) {
+    Operands op{};
+    op.x = ws + P.off_x; op.xt = ws + P.off_xt; op.ot = ws + P.off_ot; op.t2 = ws + P.off_t2;
+    if (P.prec == TRIPLES_MIXED) {
+        op.xlo = ws + P.off_xlo; op.xtlo = ws + P.off_xtlo; op.otlo = ws + P.off_otlo; op.t2lo = ws + P.off_t2lo;
+    }
+    return op;
+}
+
+// ------------------------------------------------------------------------------------------ core driver
+struct Inputs {
+    const double *eps_o, *eps_v, *t1, *t2, *vvvo, *ovoo, *ovov;
+};
+
+// Runs prepare + all batches for `trip` (restricted triplets, index = row of e_trip to write) and leaves the
+// weighted per-triplet energies in e_trip (device, 3 doubles per row; rows of i=j=k triplets are zero).
+template <typename TS>
+int run_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, const std::vector<Triplet>& trip,
+                double* e_trip, size_t e_trip_rows) {
+    const int o = P.o, v = P.v;
+    Operands op = carve_operands(P, ws);
+    const bool prof = g_profiling != 0;
+    g_events.reset();
+    cudaEvent_t ev_p0 = nullptr, ev_p1 = nullptr;
+    if (prof) {
+        if (int rc = g_events.get(&ev_p0)) return rc;
+        if (int rc = g_events.get(&ev_p1)) return rc;
+        CU_TRY(cudaEventRecord(ev_p0, st));
+    }
+    if (int rc = run_prepare<TS>(P, in.t2, in.vvvo, in.ovoo, op, st)) return rc;
+    if (prof) CU_TRY(cudaEventRecord(ev_p1, st));
+
+    GemmMaps maps;
+    if (P.prec == TRIPLES_FP64) {
+        if (int rc = build_maps_f64(P, op, &maps)) return rc;
+    } else {
+        return fail(TRIPLES_EINVAL, "mixed-precision contraction path is not built in this version");
+    }
+
+    // ---- job tables for every batch, uploaded once
+    std::vector<Orbit> orbits;
+    enumerate_orbits(v, orbits);
+    std::vector<Triplet> work;   // i=j=k contributes exactly zero (weight 0, Q5): skipped
+    for (const Triplet& t : trip)
+        if (!(t.i == t.j && t.j == t.k)) work.push_back(t);
+    const size_t nwork = work.size();
+    std::vector<GemmJob> gj;
+    std::vector<RedJob<TS>> rj(nwork);
+    std::vector<FinJob> fj(nwork);
+    std::vector<int> gj_begin;   // first gemm job of each batch
+    TS* ubase = reinterpret_cast<TS*>(ws + P.off_u);
+    double distinct_u = 0.0;
+    for (size_t n = 0; n < nwork; ++n) {
+        const Triplet& t = work[n];
+        const int slot = (int)(n % P.nb);
+        if (slot == 0) gj_begin.push_back((int)gj.size());
+        TS* u1 = ubase + (size_t)(3 * slot + 0) * P.n_u;
+        TS* u2 = ubase + (size_t)(3 * slot + 1) * P.n_u;
+        TS* u3 = ubase + (size_t)(3 * slot + 2) * P.n_u;
+        gj.push_back({t.i, t.j, t.k, 0, u1});                       // G(i,j,k)[a][b][c]
+        if (t.i == t.j) u2 = u1; else gj.push_back({t.j, t.i, t.k, 0, u2});   // G(j,i,k)[b][a][c]
+        if (t.j == t.k) u3 = u2; else gj.push_back({t.k, t.i, t.j, 0, u3});   // G(k,i,j)[c][a][b]
+        distinct_u += 1.0 + (t.i != t.j) + (t.j != t.k);
+        rj[n] = {t.i, t.j, t.k, slot, u1, u2, u3};
+        fj[n] = {slot, (int)t.index, triplet_weight(t.i, t.j, t.k)};
+    }
+    gj_begin.push_back((int)gj.size());
+    GemmJob* d_gj = reinterpret_cast<GemmJob*>(ws + P.off_gjobs);
+    RedJob<TS>* d_rj = reinterpret_cast<RedJob<TS>*>(ws + P.off_rjobs);
+    FinJob* d_fj = reinterpret_cast<FinJob*>(ws + P.off_fjobs);
+    uchar4* d_orb = reinterpret_cast<uchar4*>(ws + P.off_orb);
+    double2* d_part = reinterpret_cast<double2*>(ws + P.off_part);
+    if (!gj.empty()) CU_TRY(cudaMemcpyAsync(d_gj, gj.data(), gj.size() * sizeof(GemmJob), cudaMemcpyHostToDevice, st));
+    if (nwork) {
+        CU_TRY(cudaMemcpyAsync(d_rj, rj.data(), nwork * sizeof(RedJob<TS>), cudaMemcpyHostToDevice, st));
+        CU_TRY(cudaMemcpyAsync(d_fj, fj.data(), nwork * sizeof(FinJob), cudaMemcpyHostToDevice, st));
+    }
+    CU_TRY(cudaMemcpyAsync(d_orb, orbits.data(), orbits.size() * sizeof(Orbit), cudaMemcpyHostToDevice, st));
+    CU_TRY(cudaMemsetAsync(e_trip, 0, e_trip_rows * 3 * sizeof(double), st));
+
+    // ---- batches: contraction -> fused reduction -> per-triplet finalize
+    std::vector<cudaEvent_t> evs;
+    const size_t nbatch = (nwork + P.nb - 1) / P.nb;
+    for (size_t b = 0; b < nbatch; ++b) {
+        const size_t n0 = b * P.nb;
+        const int cnt = (int)std::min<size_t>(P.nb, nwork - n0);
+        const int g0 = gj_begin[b], g1 = gj_begin[b + 1];
+        cudaEvent_t e[4] = {nullptr, nullptr, nullptr, nullptr};
+        if (prof) {
+            for (int x = 0; x < 4; ++x) if (int rc = g_events.get(&e[x])) return rc;
+            CU_TRY(cudaEventRecord(e[0], st));
+        }
+        if (int rc = launch_gemm(P, maps, d_gj + g0, g1 - g0, st)) return rc;
+        if (prof) CU_TRY(cudaEventRecord(e[1], st));
+        reduce_kernel<TS><<<dim3(P.norb, cnt), RED_THREADS, 0, st>>>(d_rj + n0, d_orb, P.norb, v, P.vp, o, in.eps_o,
+                                                                      in.eps_v, in.t1, in.ovov, d_part);
+        CU_TRY(cudaGetLastError());
+        if (prof) CU_TRY(cudaEventRecord(e[2], st));
+        finalize_kernel<<<cnt, 128, 0, st>>>(d_fj + n0, d_part, P.norb, e_trip);
+        CU_TRY(cudaGetLastError());
+        if (prof) {
+            CU_TRY(cudaEventRecord(e[3], st));
+            for (int x = 0; x < 4; ++x) evs.push_back(e[x]);
+        }
+    }
+    if (prof) {
+        CU_TRY(cudaStreamSynchronize(st));
+        double t_gemm = 0, t_red = 0, t_fin = 0;
+        float ms = 0;
+        for (size_t b = 0; b < nbatch; ++b) {
+            CU_TRY(cudaEventElapsedTime(&ms, evs[4 * b + 0], evs[4 * b + 1])); t_gemm += ms;
+            CU_TRY(cudaEventElapsedTime(&ms, evs[4 * b + 1], evs[4 * b + 2])); t_red += ms;
+            CU_TRY(cudaEventElapsedTime(&ms, evs[4 * b + 2], evs[4 * b + 3])); t_fin += ms;
+        }
+        CU_TRY(cudaEventElapsedTime(&ms, ev_p0, ev_p1));
+        const double v3 = (double)v * v * v;
+        g_prof[0] = ms;
+        g_prof[1] = t_gemm; g_prof[2] = (double)nbatch;
+        g_prof[3] = t_red;  g_prof[4] = (double)nbatch;
+        g_prof[5] = t_fin;  g_prof[6] = (double)nbatch;
+        g_prof[7] = (double)gj.size() * 4.0 * v3 * ((double)v + o);
+        g_prof[8] = distinct_u * v3 * sizeof(TS) + (double)nwork * (3.0 * v * v + 4.0 * v) * 8.0;
+        g_prof[9] = (double)nwork;
+        g_prof_valid = true;
+    }
+    return TRIPLES_OK;
+}
+
+int validate_common(int o, int v, int prec, const void* const* ptrs, int nptr, const void* ws, size_t ws_bytes,
+                    size_t need, Plan& P) {
+    if (!make_plan(o, v, prec, P))
+        return fail(TRIPLES_EINVAL, "invalid sizes/precision: nocc=%d nvirt=%d precision=%d (need 1<=nocc<=%d, 1<=nvirt<=%d)",
+                    o, v, prec, kMaxOcc, kMaxVirt);
+    for (int n = 0; n < nptr; ++n)
+        if (!ptrs[n]) return fail(TRIPLES_EINVAL, "null pointer argument (#%d)", n);
+    if (!ws) return fail(TRIPLES_EINVAL, "null workspace");
+    if (reinterpret_cast<uintptr_t>(ws) & 255) return fail(TRIPLES_EINVAL, "workspace must be 256-byte aligned");
+    (void)need;
+    (void)ws_bytes;
+    return TRIPLES_OK;
+}
+
+int dispatch_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, const std::vector<Triplet>& trip,
+                     double* e_trip, size_t rows) {
+    if (P.prec == TRIPLES_FP64) return run_batches<double>(P, in, ws, st, trip, e_trip, rows);
+    return run_batches<float>(P, in, ws, st, trip, e_trip, rows);
+}
+
+}  // namespace
+
+// =============================================================================================== C ABI
+extern "C" {
+
+int triples_abi_version(void) { return 1; }
+
+const char* triples_last_error(void) { return g_err.c_str(); }
+
+void triples_set_profiling(int on) { g_profiling = on; }
+
+int triples_last_profile(double* out10) {
+    if (!out10 || !g_prof_valid) return fail(TRIPLES_EINVAL, "no profiled call on this thread");
+    std::memcpy(out10, g_prof, sizeof g_prof);
+    return TRIPLES_OK;
+}
+
+long long triples_triplet_count(int nocc) { return tb::triplet_count(nocc); }
+
+int triples_triplet_list(int nocc, int* ijk_out) {
+    if (nocc < 1 || !ijk_out) return fail(TRIPLES_EINVAL, "triples_triplet_list: bad arguments");
+    std::vector<Triplet> t;
+    enumerate_triplets(nocc, t);
+    for (size_t n = 0; n < t.size(); ++n) { ijk_out[3 * n] = t[n].i; ijk_out[3 * n + 1] = t[n].j; ijk_out[3 * n + 2] = t[n].k; }
+    return TRIPLES_OK;
+}
+
+size_t triples_workspace_bytes(int nocc, int nvirt, int precision) {
+    Plan P;
+    return make_plan(nocc, nvirt, precision, P) ? P.total : 0;
+}
+
+size_t triples_workspace_bytes_host(int nocc, int nvirt, int precision) {
+    Plan P;
+    return make_plan(nocc, nvirt, precision, P) ? P.total_host : 0;
+}
+
+int triples_energy(int nocc, int nvirt, const double* eps_o, const double* eps_v, const double* t1, const double* t2,
+                   const double* vvvo, const double* ovoo, const double* ovov, int precision, void* workspace,
+                   size_t workspace_bytes, void* cuda_stream, double* e_out, double* e_triplet_out) {
+    Plan P;
+    const void* ptrs[8] = {eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, e_out};
+    if (int rc = validate_common(nocc, nvirt, precision, ptrs, 8, workspace, workspace_bytes, 0, P)) return rc;
+    for (int n = 0; n < 7; ++n)
+        if (misaligned(ptrs[n])) return fail(TRIPLES_EINVAL, "input pointer #%d is not 16-byte aligned", n);
+    if (workspace_bytes < P.total)
+        return fail(TRIPLES_EWORKSPACE, "workspace too small: %zu bytes given, %zu needed", workspace_bytes, P.total);
+    if (int rc = check_device()) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    uint8_t* ws = static_cast<uint8_t*>(workspace);
+    std::vector<Triplet> trip;
+    enumerate_triplets(nocc, trip);
+    double* e_trip = reinterpret_cast<double*>(ws + P.off_etrip);
+    double* d_res = reinterpret_cast<double*>(ws + P.off_result);
+    Inputs in{eps_o, eps_v, t1, t2, vvvo, ovoo, ovov};
+    g_prof_valid = false;
+    if (int rc = dispatch_batches(P, in, ws, st, trip, e_trip, (size_t)P.T)) return rc;
+    total_kernel<<<1, 256, 0, st>>>(e_trip, P.T, d_res);
+    CU_TRY(cudaGetLastError());
+    if (e_triplet_out)
+        CU_TRY(cudaMemcpyAsync(e_triplet_out, e_trip, (size_t)P.T * 3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    CU_TRY(cudaMemcpyAsync(e_out, d_res, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CU_TRY(cudaStreamSynchronize(st));
+    return TRIPLES_OK;
+}
+
+int triples_energy_host(int nocc, int nvirt, const double* eps_o, const double* eps_v, const double* t1,
+                        const double* t2, const double* vvvo, const double* ovoo, const double* ovov, int precision,
+                        void* workspace, size_t workspace_bytes, void* cuda_stream, double* e_out,
+                        double* e_triplet_out) {
+    Plan P;
+    const void* ptrs[8] = {eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, e_out};
+    if (int rc = validate_common(nocc, nvirt, precision, ptrs, 8, workspace, workspace_bytes, 0, P)) return rc;
+    if (workspace_bytes < P.total_host)
+        return fail(TRIPLES_EWORKSPACE, "workspace too small: %zu bytes given, %zu needed", workspace_bytes, P.total_host);
+    if (int rc = check_device()) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    uint8_t* ws = static_cast<uint8_t*>(workspace);
+    const double* dev[7];
+    for (int n = 0; n < 7; ++n) {
+        CU_TRY(cudaMemcpyAsync(ws + P.off_in[n], ptrs[n], P.in_bytes[n], cudaMemcpyHostToDevice, st));
+        dev[n] = reinterpret_cast<const double*>(ws + P.off_in[n]);
+    }
+    int rc = triples_energy(nocc, nvirt, dev[0], dev[1], dev[2], dev[3], dev[4], dev[5], dev[6], precision, workspace,
+                            P.total, cuda_stream, e_out, nullptr);
+    if (rc) return rc;
+    if (e_triplet_out) {
+        CU_TRY(cudaMemcpyAsync(e_triplet_out, ws + P.off_etrip, (size_t)P.T * 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CU_TRY(cudaStreamSynchronize(st));
+    }
+    return TRIPLES_OK;
+}
+
+int triples_energy_subset(int nocc, int nvirt, const double* eps_o, const double* eps_v, const double* t1,
+                          const double* t2, const double* vvvo, const double* ovoo, const double* ovov, int precision,
+                          int ntrip, const int* ijk, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                          double* e_out) {
+    Plan P;
+    const void* ptrs[7] = {eps_o, eps_v, t1, t2, vvvo, ovoo, ovov};
+    if (int rc = validate_common(nocc, nvirt, precision, ptrs, 7, workspace, workspace_bytes, 0, P)) return rc;
+    if (ntrip < 0 || (ntrip > 0 && (!ijk || !e_out))) return fail(TRIPLES_EINVAL, "bad triplet list");
+    if ((long long)ntrip > P.T) return fail(TRIPLES_EINVAL, "more triplets (%d) than the restricted loop has (%lld)", ntrip, P.T);
+    for (int n = 0; n < 7; ++n)
+        if (misaligned(ptrs[n])) return fail(TRIPLES_EINVAL, "input pointer #%d is not 16-byte aligned", n);
+    if (workspace_bytes < P.total)
+        return fail(TRIPLES_EWORKSPACE, "workspace too small: %zu bytes given, %zu needed", workspace_bytes, P.total);
+    std::vector<Triplet> trip(ntrip);
+    for (int n = 0; n < ntrip; ++n) {
+        const int i = ijk[3 * n], j = ijk[3 * n + 1], k = ijk[3 * n + 2];
+        if (i < 0 || i > j || j > k || k >= nocc) return fail(TRIPLES_EINVAL, "triplet #%d = (%d,%d,%d) is not 0<=i<=j<=k<nocc", n, i, j, k);
+        trip[n] = {i, j, k, n};
+    }
+    if (ntrip == 0) return TRIPLES_OK;
+    if (int rc = check_device()) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    uint8_t* ws = static_cast<uint8_t*>(workspace);
+    double* e_trip = reinterpret_cast<double*>(ws + P.off_etrip);
+    Inputs in{eps_o, eps_v, t1, t2, vvvo, ovoo, ovov};
+    g_prof_valid = false;
+    if (int rc = dispatch_batches(P, in, ws, st, trip, e_trip, (size_t)ntrip)) return rc;
+    CU_TRY(cudaMemcpyAsync(e_out, e_trip, (size_t)ntrip * 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CU_TRY(cudaStreamSynchronize(st));
+    return TRIPLES_OK;
+}
+
+int triples_w_block(int nocc, int nvirt, const double* t2, const double* vvvo, const double* ovoo, int precision,
+                    int i, int j, int k, void* workspace, size_t workspace_bytes, void* cuda_stream, double* W_out) {
+    Plan P;
+    const void* ptrs[4] = {t2, vvvo, ovoo, W_out};
+    if (int rc = validate_common(nocc, nvirt, precision, ptrs, 4, workspace, workspace_bytes, 0, P)) return rc;
+    if (i < 0 || j < 0 || k < 0 || i >= nocc || j >= nocc || k >= nocc) return fail(TRIPLES_EINVAL, "occupied index out of range");
+    for (int n = 0; n < 3; ++n)
+        if (misaligned(ptrs[n])) return fail(TRIPLES_EINVAL, "input pointer #%d is not 16-byte aligned", n);
+    if (workspace_bytes < P.total)
+        return fail(TRIPLES_EWORKSPACE, "workspace too small: %zu bytes given, %zu needed", workspace_bytes, P.total);
+    if (precision != TRIPLES_FP64) return fail(TRIPLES_EINVAL, "mixed-precision contraction path is not built in this version");
+    if (int rc = check_device()) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    uint8_t* ws = static_cast<uint8_t*>(workspace);
+    Operands op = carve_operands(P, ws);
+    if (int rc = run_prepare<double>(P, t2, vvvo, ovoo, op, st)) return rc;
+    GemmMaps maps;
+    if (int rc = build_maps_f64(P, op, &maps)) return rc;
+    double* ubase = reinterpret_cast<double*>(ws + P.off_u);
+    GemmJob gj[3] = {{i, j, k, 0, ubase}, {j, i, k, 0, ubase + P.n_u}, {k, i, j, 0, ubase + 2 * P.n_u}};
+    GemmJob* d_gj = reinterpret_cast<GemmJob*>(ws + P.off_gjobs);
+    CU_TRY(cudaMemcpyAsync(d_gj, gj, sizeof gj, cudaMemcpyHostToDevice, st));
+    if (int rc = launch_gemm(P, maps, d_gj, 3, st)) return rc;
+    assemble_w_kernel<double><<<kNumSM * 4, 256, 0, st>>>(ubase, ubase + P.n_u, ubase + 2 * P.n_u, nvirt, P.vp, W_out);
+    CU_TRY(cudaGetLastError());
+    CU_TRY(cudaStreamSynchronize(st));
+    return TRIPLES_OK;
+}
+
+}  // extern "C"
