@@ -137,6 +137,10 @@ int triples_w_block(int nocc, int nvirt,
 int triples_last_profile(double* out10);
 void triples_set_profiling(int on);
 
+/* Number of CUDA kernels the calling thread's last compute call (triples_energy / _host / _subset / _w_block)
+ * launched (repack + contraction + reduction + finalize + total). */
+long long triples_last_launch_count(void);
+
 /* Thread-local message for the last non-OK status ("" if none). Never NULL. */
 const char* triples_last_error(void);
 

@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     triples_energy,
     triples_energy_host,
     triples_energy_subset,
+    triples_last_launch_count,
     triples_last_profile,
     triples_set_profiling,
     triples_triplet_count,

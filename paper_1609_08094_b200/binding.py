@@ -41,6 +41,7 @@ def lib() -> ctypes.CDLL:
         L.triples_set_profiling.restype = None
         L.triples_last_profile.argtypes = [dp]
         L.triples_last_profile.restype = ctypes.c_int
+        L.triples_last_launch_count.restype = ctypes.c_longlong
         L.triples_triplet_count.argtypes = [ctypes.c_int]
         L.triples_triplet_count.restype = ctypes.c_longlong
         L.triples_triplet_list.argtypes = [ctypes.c_int, ip]
@@ -133,6 +134,10 @@ def triples_last_profile() -> dict:
     keys = ("prepare_ms", "contraction_ms", "contraction_launches", "reduction_ms", "reduction_launches",
             "other_ms", "other_launches", "contraction_flops", "reduction_bytes", "triplets")
     return dict(zip(keys, [float(x) for x in out]))
+
+
+def triples_last_launch_count() -> int:
+    return int(lib().triples_last_launch_count())
 
 
 def triples_energy(nocc, nvirt, eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, precision, workspace, stream=None,

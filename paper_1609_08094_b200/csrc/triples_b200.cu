@@ -25,6 +25,7 @@ thread_local std::string g_err;
 thread_local double g_prof[10];
 thread_local bool g_prof_valid = false;
 thread_local int g_profiling = 0;
+thread_local long long g_launches = 0;   // kernels launched by the calling thread's last compute call
 
 int fail(int code, const char* fmt, ...) {
     char buf[512];
@@ -122,6 +123,7 @@ int launch_gemm_f64(const GemmMaps& maps, const GemmJob* jobs, int njobs, const 
     dim3 grid(P.mtiles * P.ntiles, njobs);
     kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(maps, jobs, P.v, P.vp, P.o, P.mtiles);
     CU_TRY(cudaGetLastError());
+    ++g_launches;
     return TRIPLES_OK;
 }
 
@@ -184,6 +186,7 @@ int run_prepare(const Plan& P, const double* t2, const double* vvvo, const doubl
         CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
         kern<<<(unsigned)((R + RB - 1) / RB), 256, smem, st>>>(vvvo, v, P.vp, o, RB, (TO*)op.x, (TO*)op.xlo);
         CU_TRY(cudaGetLastError());
+        ++g_launches;
     }
     {   // XT (and its low part)
         dim3 grid((v + 31) / 32, (v + 31) / 32, 1);
@@ -194,13 +197,16 @@ int run_prepare(const Plan& P, const double* t2, const double* vvvo, const doubl
             transpose_planes_kernel<TO><<<grid, 256, 0, st>>>((const TO*)op.x + sl, v, P.vp, (TO*)op.xt + sl);
             if (split)
                 transpose_planes_kernel<TO><<<grid, 256, 0, st>>>((const TO*)op.xlo + sl, v, P.vp, (TO*)op.xtlo + sl);
+            g_launches += split ? 2 : 1;
         }
         CU_TRY(cudaGetLastError());
     }
     pack_ot_kernel<TO><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.op, (TO*)op.ot, (TO*)op.otlo);
     CU_TRY(cudaGetLastError());
+    ++g_launches;
     pack_t2_kernel<TO><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vp, (TO*)op.t2, (TO*)op.t2lo);
     CU_TRY(cudaGetLastError());
+    ++g_launches;
     return TRIPLES_OK;
 }
 
@@ -301,9 +307,11 @@ int run_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, c
         reduce_kernel<TS><<<dim3(P.norb, cnt), RED_THREADS, 0, st>>>(d_rj + n0, d_orb, P.norb, v, P.vp, o, in.eps_o,
                                                                       in.eps_v, in.t1, in.ovov, d_part);
         CU_TRY(cudaGetLastError());
+        ++g_launches;
         if (prof) CU_TRY(cudaEventRecord(e[2], st));
         finalize_kernel<<<cnt, 128, 0, st>>>(d_fj + n0, d_part, P.norb, e_trip);
         CU_TRY(cudaGetLastError());
+        ++g_launches;
         if (prof) {
             CU_TRY(cudaEventRecord(e[3], st));
             for (int x = 0; x < 4; ++x) evs.push_back(e[x]);
@@ -359,6 +367,8 @@ extern "C" {
 
 int triples_abi_version(void) { return 1; }
 
+long long triples_last_launch_count(void) { return g_launches; }
+
 const char* triples_last_error(void) { return g_err.c_str(); }
 
 void triples_set_profiling(int on) { g_profiling = on; }
@@ -408,9 +418,11 @@ int triples_energy(int nocc, int nvirt, const double* eps_o, const double* eps_v
     double* d_res = reinterpret_cast<double*>(ws + P.off_result);
     Inputs in{eps_o, eps_v, t1, t2, vvvo, ovoo, ovov};
     g_prof_valid = false;
+    g_launches = 0;
     if (int rc = dispatch_batches(P, in, ws, st, trip, e_trip, (size_t)P.T)) return rc;
     total_kernel<<<1, 256, 0, st>>>(e_trip, P.T, d_res);
     CU_TRY(cudaGetLastError());
+    ++g_launches;
     if (e_triplet_out)
         CU_TRY(cudaMemcpyAsync(e_triplet_out, e_trip, (size_t)P.T * 3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
     CU_TRY(cudaMemcpyAsync(e_out, d_res, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -471,6 +483,7 @@ int triples_energy_subset(int nocc, int nvirt, const double* eps_o, const double
     double* e_trip = reinterpret_cast<double*>(ws + P.off_etrip);
     Inputs in{eps_o, eps_v, t1, t2, vvvo, ovoo, ovov};
     g_prof_valid = false;
+    g_launches = 0;
     if (int rc = dispatch_batches(P, in, ws, st, trip, e_trip, (size_t)ntrip)) return rc;
     CU_TRY(cudaMemcpyAsync(e_out, e_trip, (size_t)ntrip * 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CU_TRY(cudaStreamSynchronize(st));
@@ -492,6 +505,7 @@ int triples_w_block(int nocc, int nvirt, const double* t2, const double* vvvo, c
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     uint8_t* ws = static_cast<uint8_t*>(workspace);
     Operands op = carve_operands(P, ws);
+    g_launches = 0;
     if (int rc = run_prepare<double>(P, t2, vvvo, ovoo, op, st)) return rc;
     GemmMaps maps;
     if (int rc = build_maps_f64(P, op, &maps)) return rc;
@@ -502,6 +516,7 @@ int triples_w_block(int nocc, int nvirt, const double* t2, const double* vvvo, c
     if (int rc = launch_gemm(P, maps, d_gj, 3, st)) return rc;
     assemble_w_kernel<double><<<kNumSM * 4, 256, 0, st>>>(ubase, ubase + P.n_u, ubase + 2 * P.n_u, nvirt, P.vp, W_out);
     CU_TRY(cudaGetLastError());
+    ++g_launches;
     CU_TRY(cudaStreamSynchronize(st));
     return TRIPLES_OK;
 }

@@ -1,0 +1,266 @@
+"""GPU parity tests: the CUDA path, called through the C ABI (ctypes binding), against the CPU oracle on the
+same seeded inputs.  Tolerances are BASELINE.json's: relative error <= 1e-10 in FP64 (<= 1e-5 mixed), asserted
+on E(T), E[4] and E[5] separately (E[5] is invisible in E(T) with the generator's t1).
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_1609_08094_b200 as tb
+from oracle import oracle
+from paper_1609_08094_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL = {tb.FP64: 1e-10, tb.MIXED: 1e-5}
+NAMES = ("eps_o", "eps_v", "t1", "t2", "vvvo", "ovoo", "ovov")
+
+
+def to_dev(inp):
+    return [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in inp.arrays()]
+
+
+def workspace(o, v, prec, host=False):
+    n = tb.triples_workspace_bytes_host(o, v, prec) if host else tb.triples_workspace_bytes(o, v, prec)
+    return torch.empty(n, dtype=torch.uint8, device="cuda")
+
+
+def rel(a, b):
+    return abs(a - b) / max(abs(b), 1e-300)
+
+
+def gpu_energy(inp, prec=tb.FP64, with_triplets=False):
+    o, v = inp.nocc, inp.nvirt
+    d = to_dev(inp)
+    ws = workspace(o, v, prec)
+    et = torch.zeros((tb.triples_triplet_count(o), 3), dtype=torch.float64, device="cuda") if with_triplets else None
+    E = tb.triples_energy(o, v, *d, prec, ws, e_triplet_out=et)
+    return (E, et.cpu().numpy()) if with_triplets else E
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# contraction stage, elementwise: W_ijk^abc of Eq. (2.2.2)-(2.2.3) against the oracle's loops
+# sizes span several CTA tiles (BM = 40/80/120, BN = 128/192/256) and ragged tails (odd v, odd o)
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("o,v,naux,ijk", [
+    (3, 5, 9, (0, 1, 2)), (3, 5, 9, (2, 0, 1)), (3, 5, 9, (1, 1, 0)), (3, 5, 9, (2, 2, 2)),
+    (4, 17, 20, (3, 0, 2)), (5, 41, 50, (4, 2, 0)), (3, 50, 40, (0, 1, 2)), (6, 96, 60, (5, 1, 3)),
+    (4, 130, 50, (1, 3, 2)), (8, 40, 120, (7, 3, 5)), (17, 24, 30, (16, 0, 9)),
+])
+def test_w_block_elementwise(o, v, naux, ijk):
+    inp = synth.make_inputs(o, v, naux, seed=3)
+    d = to_dev(inp)
+    ws = workspace(o, v, tb.FP64)
+    W = torch.full((v, v, v), float("nan"), dtype=torch.float64, device="cuda")
+    tb.triples_w_block(o, v, d[3], d[4], d[5], tb.FP64, *ijk, ws, W)
+    Wo = oracle.w_block(o, v, inp.t2, inp.vvvo, inp.ovoo, *ijk)
+    err = np.abs(W.cpu().numpy() - Wo).max()
+    assert err <= 1e-13 * np.abs(Wo).max(), f"max abs err {err:.3e} vs scale {np.abs(Wo).max():.3e}"
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# full E(T), E[4], E[5] and every per-triplet energy against the oracle's restricted loops
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("o,v,naux,t1_sigma", [
+    (1, 6, 8, 0.3), (2, 1, 4, 0.3), (2, 3, 5, 0.3), (3, 5, 9, 0.3), (2, 8, 12, 0.3), (4, 16, 30, 0.3), (3, 17, 30, 0.3),
+    (5, 41, 60, 0.3), (6, 24, 40, 1.0), (7, 33, 40, 1e-3),
+])
+def test_energy_small_cases(o, v, naux, t1_sigma):
+    inp = synth.make_inputs(o, v, naux, seed=1, t1_sigma=t1_sigma)
+    (E, et) = gpu_energy(inp, with_triplets=True)
+    (Eo, et_o) = oracle.energy_restricted(o, v, *inp.arrays(), with_triplets=True)
+    scale = max(abs(Eo[1]), 1e-300)
+    if o == 1 or v == 1:                       # degenerate sizes: E(T) = 0 exactly
+        assert all(abs(x) <= 1e-25 for x in E) and all(abs(x) <= 1e-25 for x in Eo)
+        return
+    for n in range(3):
+        assert abs(E[n] - Eo[n]) <= TOL[tb.FP64] * max(abs(Eo[n]), 1e-3 * scale), (n, E, Eo)
+    assert np.abs(et - et_o).max() <= TOL[tb.FP64] * np.abs(et_o).max()
+
+
+def test_tiny_config_full_parity():
+    """BASELINE.json configs[0]: nocc=8, nvirt=40, naux=120, seed 0 -- the case the oracle finishes in seconds."""
+    inp = synth.make_config("tiny")
+    (E, et) = gpu_energy(inp, with_triplets=True)
+    (Eo, et_o) = oracle.energy_restricted(inp.nocc, inp.nvirt, *inp.arrays(), with_triplets=True)
+    assert E[0] < 0 and Eo[0] < 0                                          # reading Q1: E(T) < 0
+    for n in range(3):
+        assert rel(E[n], Eo[n]) <= TOL[tb.FP64], (n, E, Eo)
+    assert np.abs(et - et_o).max() <= TOL[tb.FP64] * np.abs(et_o).max()
+    diag = [n for n, (i, j, k) in enumerate(synth.triplet_list(inp.nocc)) if i == j == k]
+    assert np.all(et[diag] == 0.0)                                          # i=j=k contribute exactly zero (Q5)
+    assert rel(et[:, 0].sum(), E[0]) <= 1e-13                               # sum of per-triplet energies = E(T)
+
+
+def test_tiny_config_large_t1_pins_e5():
+    """Second input set with t1 ~ N(0,1) so that E[5] is of the order of E[4]."""
+    inp = synth.make_config("tiny", seed=5, t1_sigma=1.0)
+    E = gpu_energy(inp)
+    Eo = oracle.energy_restricted(inp.nocc, inp.nvirt, *inp.arrays())
+    assert abs(Eo[2]) > 1e-3 * abs(Eo[1])
+    for n in range(3):
+        assert rel(E[n], Eo[n]) <= TOL[tb.FP64], (n, E, Eo)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# BASELINE.json configs[1..4] at full size: sampled triplets (oracle: numpy restatement, one triplet at a time)
+# ------------------------------------------------------------------------------------------------------------------
+SAMPLES = {"small": 32, "medium": 32, "large": 10, "largest": 8}
+
+
+@pytest.mark.parametrize("name", ["small", "medium", "large", "largest"])
+def test_config_sampled_triplets(name):
+    o, v, naux = synth.CONFIGS[name]
+    free, _ = torch.cuda.mem_get_info()
+    need = tb.triples_workspace_bytes(o, v, tb.FP64) + 8 * v ** 3 * o * 1.2
+    if free < need:
+        pytest.skip(f"{name}: needs {need/1e9:.0f} GB of device memory, {free/1e9:.0f} GB free")
+    d = synth.make_inputs_device(o, v, naux, seed=0)
+    args = [d[k] for k in NAMES]
+    trips = synth.sample_triplets(o, SAMPLES[name], seed=0)
+    ws = workspace(o, v, tb.FP64)
+    e_gpu = tb.triples_energy_subset(o, v, *args, tb.FP64, trips, ws)
+    # host copies of what the oracle needs: small tensors and the vvvo slices of the sampled occupied indices
+    host = {k: d[k].cpu().numpy() for k in ("eps_o", "eps_v", "t1", "t2", "ovoo", "ovov")}
+    slices = {}
+    for r in sorted({x for t in trips for x in t}):
+        slices[r] = d["vvvo"][:, :, :, r].contiguous().cpu().numpy()
+    # spot-check the device-generated integrals against the B factors on the host (generator only)
+    B = d["B_host"]
+    rng = np.random.default_rng(0)
+    for _ in range(20):
+        a, b, c = rng.integers(0, v, 3)
+        r = sorted(slices)[int(rng.integers(0, len(slices)))]
+        ref = float(B[:, o + a, o + b] @ B[:, o + c, r])
+        assert abs(slices[r][a, b, c] - ref) <= 1e-12 * max(1.0, abs(ref))
+    e_or = oracle.energy_subset_numpy(host["eps_o"], host["eps_v"], host["t1"], host["t2"], None, host["ovoo"],
+                                      host["ovov"], trips, vvvo_slices=slices)
+    for n, t in enumerate(trips):
+        if t[0] == t[1] == t[2]:
+            assert np.all(e_gpu[n] == 0.0) and np.abs(e_or[n]).max() <= 1e-12 * np.abs(e_or[:, 1]).max()
+            continue
+        s4 = abs(e_or[n, 1])
+        assert abs(e_gpu[n, 1] - e_or[n, 1]) <= TOL[tb.FP64] * s4, (t, e_gpu[n], e_or[n])
+        assert abs(e_gpu[n, 0] - e_or[n, 0]) <= TOL[tb.FP64] * s4, (t, e_gpu[n], e_or[n])
+        # E[5] per triplet: absolute error bounded relative to the triplet's own scale |e4|*1e-10 or |e5|*1e-8
+        assert abs(e_gpu[n, 2] - e_or[n, 2]) <= max(TOL[tb.FP64] * s4, 1e-8 * abs(e_or[n, 2])), (t, e_gpu[n], e_or[n])
+
+
+@pytest.mark.parametrize("name", ["small", "medium"])
+def test_config_full_run_properties(name):
+    """Full E(T) in the launch configuration bench.py times: properties that hold at any size."""
+    o, v, naux = synth.CONFIGS[name]
+    d = synth.make_inputs_device(o, v, naux, seed=0)
+    args = [d[k] for k in NAMES]
+    ws = workspace(o, v, tb.FP64)
+    T = tb.triples_triplet_count(o)
+    et = torch.zeros((T, 3), dtype=torch.float64, device="cuda")
+    E = tb.triples_energy(o, v, *args, tb.FP64, ws, e_triplet_out=et)
+    et = et.cpu().numpy()
+    assert E[0] < 0 and E[1] < 0
+    assert rel(et[:, 0].sum(), E[0]) <= 1e-13 and rel(et[:, 1].sum(), E[1]) <= 1e-13
+    trip = synth.triplet_list(o)
+    for n, (i, j, k) in enumerate(trip):
+        if i == j == k:
+            assert np.all(et[n] == 0.0)
+        else:
+            assert et[n, 1] < 0.0                # P6: e4_ijk <= 0 for every triplet when all D < 0
+    # the sampled subset entry point returns the same numbers as the full run, bit for bit
+    sample = synth.sample_triplets(o, 12, seed=1)
+    sub = tb.triples_energy_subset(o, v, *args, tb.FP64, sample, ws)
+    idx = [trip.index(t) for t in sample]
+    assert np.array_equal(sub, et[idx])
+    # run-to-run bitwise determinism (no atomics anywhere)
+    E2 = tb.triples_energy(o, v, *args, tb.FP64, ws)
+    assert E2 == E
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# invariants on the GPU path itself, degenerate inputs, host entry point, error behaviour
+# ------------------------------------------------------------------------------------------------------------------
+def test_relabelling_invariance_on_gpu():
+    inp = synth.make_inputs(5, 21, 30, seed=7, t1_sigma=0.5)
+    rng = np.random.default_rng(1)
+    po, pv = rng.permutation(inp.nocc), rng.permutation(inp.nvirt)
+    perm = synth.TriplesInputs(
+        inp.nocc, inp.nvirt, inp.eps_o[po], inp.eps_v[pv], np.ascontiguousarray(inp.t1[po][:, pv]),
+        np.ascontiguousarray(inp.t2[po][:, po][:, :, pv][:, :, :, pv]),
+        np.ascontiguousarray(inp.vvvo[pv][:, pv][:, :, pv][:, :, :, po]),
+        np.ascontiguousarray(inp.ovoo[po][:, pv][:, :, po][:, :, :, po]),
+        np.ascontiguousarray(inp.ovov[po][:, pv][:, :, po][:, :, :, pv]))
+    E, Ep = gpu_energy(inp), gpu_energy(perm)
+    for n in range(3):
+        assert rel(Ep[n], E[n]) <= 1e-12
+
+
+def test_zero_inputs_and_scaling_on_gpu():
+    inp = synth.make_inputs(4, 12, 20, seed=2, t1_sigma=0.0)
+    E = gpu_energy(inp)
+    z = synth.TriplesInputs(inp.nocc, inp.nvirt, inp.eps_o, inp.eps_v, inp.t1, inp.t2, inp.vvvo * 0, inp.ovoo * 0,
+                            inp.ovov * 0)
+    assert gpu_energy(z) == (0.0, 0.0, 0.0)
+    lam = 1.7
+    s = synth.TriplesInputs(inp.nocc, inp.nvirt, inp.eps_o, inp.eps_v, inp.t1, inp.t2 * lam, inp.vvvo, inp.ovoo,
+                            inp.ovov)
+    Es = gpu_energy(s)
+    assert rel(Es[0], lam * lam * E[0]) <= 1e-12 and abs(Es[2]) == 0.0 and abs(E[2]) == 0.0
+
+
+def test_host_entry_point_matches_device_entry_point():
+    inp = synth.make_inputs(6, 40, 50, seed=4, t1_sigma=0.1)
+    o, v = inp.nocc, inp.nvirt
+    E = gpu_energy(inp)
+    ws = workspace(o, v, tb.FP64, host=True)
+    T = tb.triples_triplet_count(o)
+    et = np.zeros((T, 3))
+    Eh = tb.triples_energy_host(o, v, *[np.ascontiguousarray(a) for a in inp.arrays()], tb.FP64, ws, e_triplet_out=et)
+    assert Eh == E
+    assert rel(et[:, 0].sum(), E[0]) <= 1e-13
+    assert tb.triples_last_launch_count() > 0
+
+
+def test_error_codes():
+    inp = synth.make_inputs(3, 8, 10, seed=0)
+    o, v = inp.nocc, inp.nvirt
+    d = to_dev(inp)
+    ws = workspace(o, v, tb.FP64)
+    with pytest.raises(tb.TriplesError) as e:
+        tb.triples_energy(o, v, *d, tb.FP64, ws[: ws.numel() // 2])
+    assert e.value.status == 2                                              # EWORKSPACE
+    with pytest.raises(tb.TriplesError) as e:
+        tb.triples_energy(o, v, *d, 5, ws)
+    assert e.value.status == 1                                              # EINVAL: unknown precision
+    big = torch.zeros(d[3].numel() + 1, dtype=torch.float64, device="cuda")
+    mis = big[1:].view(d[3].shape)                                          # 8-byte aligned only
+    mis.copy_(d[3])
+    with pytest.raises(tb.TriplesError) as e:
+        tb.triples_energy(o, v, d[0], d[1], d[2], mis, d[4], d[5], d[6], tb.FP64, ws)
+    assert e.value.status == 1
+    with pytest.raises(tb.TriplesError) as e:
+        tb.triples_energy_subset(o, v, *d, tb.FP64, [(2, 1, 0)], ws)         # not i<=j<=k
+    assert e.value.status == 1
+    # the library is still usable after errors
+    E = tb.triples_energy(o, v, *d, tb.FP64, ws)
+    Eo = oracle.energy_restricted(o, v, *inp.arrays())
+    assert rel(E[0], Eo[0]) <= TOL[tb.FP64]
+
+
+def test_profile_and_launch_count():
+    inp = synth.make_config("tiny")
+    o, v = inp.nocc, inp.nvirt
+    d = to_dev(inp)
+    ws = workspace(o, v, tb.FP64)
+    tb.triples_set_profiling(True)
+    try:
+        tb.triples_energy(o, v, *d, tb.FP64, ws)
+        p = tb.triples_last_profile()
+    finally:
+        tb.triples_set_profiling(False)
+    T = tb.triples_triplet_count(o)
+    assert p["triplets"] == T - o
+    # executed flops: 12v^4 + 12ov^3 per triplet, one of the three GEMMs skipped when i=j or j=k
+    full = 12 * v ** 4 + 12 * o * v ** 3
+    n_pair = sum(1 for (i, j, k) in synth.triplet_list(o) if (i == j) != (j == k))
+    assert p["contraction_flops"] == pytest.approx((T - o) * full - n_pair * full / 3, rel=1e-12)
+    assert p["contraction_ms"] > 0 and p["reduction_ms"] > 0
+    assert tb.triples_last_launch_count() >= 3 * p["contraction_launches"] + 1
