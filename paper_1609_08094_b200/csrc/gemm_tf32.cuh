@@ -1,0 +1,221 @@
+// gemm_tf32.cuh -- mixed-precision contraction kernel (S2+S3 of DESIGN.md): TMA -> swizzled smem -> tcgen05.mma
+// (kind::tf32, 3xTF32 split) with FP32 accumulators in TMEM.
+//
+// The paper's mixed precision runs "only the construction of the triples amplitudes" through
+// sgemm.  B200 has no FP32 tensor path; an FP32-accurate product is recovered from three TF32 products of the
+// round-to-nearest hi/lo split made by prepare.cuh (Q13):   x*y ~= xh*yh + xh*yl + xl*yh.
+//
+// Same "G job" (p,q,r) as gemm_f64.cuh, computed TRANSPOSED so that the long flattened (b,c) index is the MMA's
+// M dimension (128 TMEM lanes per CTA, no padding waste for any v) and the virtual index a is its N dimension:
+//
+//   G(p,q,r)[a,(b,c)] = sum_d XK_r [(b,c),d] T2A[p,q][a,d]  + sum_d XKT_q[(b,c),d] T2A[p,r][a,d]     (Eq. (2.2.2))
+//                     + sum_l T2K_q[(b,c),l] OtA[r,p][a,l]  + sum_l T2KT_r[(b,c),l] OtA[q,p][a,l]
+//
+// Operands are K-major FP32 arrays (prepare.cuh): XK[r][b][c][d] = (db|cr), XKT[r][b][c][d] = XK[r][c][b][d],
+// T2A[p][q][a][d] = t2, OtA[r][p][a][l] = -(pa|lr), T2K[q][b][c][l] = t2[q,l,b,c], T2KT[r][b][c][l] = t2[l,r,b,c];
+// the c index has vp rows per b (row v is zero when v is odd) so that U keeps the pitch the reduction expects.
+//
+// One CTA (persistent, one per SM) walks work items (job, m-tile of 128 (b,c) rows, n-tile of BN a-columns):
+//   warp 0    : TMA producer   (K chunks of 32 floats = one 128-byte swizzled row per operand row; hi and lo tiles)
+//   warp 1    : MMA issuer     (one lane; per K chunk: 4 k-steps of lo*hi and hi*lo, then 4 k-steps of hi*hi)
+//   warp 2    : TMEM allocator (512 columns = two 128 x 256 FP32 buffers)
+//   warps 4-11: accumulators   (tcgen05.ld of every finished chain, FP32 round-to-nearest adds in registers,
+//                               coalesced FP32 stores of U[a][(b,c)] at the end of the tile)
+//
+// Why the running sum lives in registers and not in TMEM: the tensor core adds each MMA's result to its accumulator
+// with truncation, so one long accumulation chain is biased towards zero by ~(number of MMAs) * 2^-25 (measured:
+// -3.4e-6 relative on W at v = 240, i.e. 7e-6 on E(T), growing with v).  A TMEM buffer therefore only ever holds a
+// short chain (TF_CHAIN K chunks, started with accumulate = 0, the small lo*hi / hi*lo terms first); finished chains
+// are added with FADD.RN by the accumulator warps while the tensor core fills the other buffer.
+#pragma once
+#include "gemm_f64.cuh"   // GemmJob
+#include "ptx.cuh"
+
+namespace tb {
+
+struct alignas(64) Tf32Maps {
+    // index 0 = hi part, 1 = lo part
+    CUtensorMap xk[2];    // (d, n=(b,c'), r)      box (32, 128, 1)   M side, virtual segment 1
+    CUtensorMap xkt[2];   // (d, n, r)             box (32, 128, 1)   M side, virtual segment 2
+    CUtensorMap t2k[2];   // (l, n, q)             box (32, 128, 1)   M side, occupied segment 3
+    CUtensorMap t2kt[2];  // (l, n, r)             box (32, 128, 1)   M side, occupied segment 4
+    CUtensorMap t2a[2];   // (d, a, p*o+q)         box (32, BN, 1)    N side, virtual segments
+    CUtensorMap ota[2];   // (l, a, r*o+p)         box (32, BN, 1)    N side, occupied segments
+};
+
+constexpr int TF_BM = 128;            // (b,c) rows per CTA tile = TMEM lanes
+constexpr int TF_BK = 32;             // floats per K chunk (128-byte rows)
+constexpr int TF_THREADS = 384;         // 4 service warps + 8 accumulator warps
+constexpr int TF_CHAIN = 1;             // K chunks per TMEM accumulation chain
+constexpr int TF_TMEM_COLS = 512;
+constexpr int TF_MAX_STAGES = 4;
+constexpr int TF_SMEM_LIMIT = 227 * 1024;
+
+__host__ __device__ constexpr int tf32_stage_bytes(int bn) { return 2 * TF_BM * 128 + 2 * bn * 128; }
+// stages that fit (>= 2 for every bn <= 256), capped; the dynamic smem request is always > half an SM's shared
+// memory so that exactly one CTA is resident per SM (it owns all 512 TMEM columns).
+__host__ __device__ constexpr int tf32_stages(int bn) {
+    int s = (TF_SMEM_LIMIT - 2048) / tf32_stage_bytes(bn);
+    return s > TF_MAX_STAGES ? TF_MAX_STAGES : s;
+}
+__host__ __device__ constexpr int tf32_smem_bytes(int bn) { return tf32_stages(bn) * tf32_stage_bytes(bn) + 2048; }
+
+__global__ void __launch_bounds__(TF_THREADS, 1)
+gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restrict__ jobs, int njobs, int v, int vp,
+                 int o, int mtiles, int ntiles, int bn) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    const int stages = tf32_stages(bn);
+    const int stage_bytes = tf32_stage_bytes(bn);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + stages * stage_bytes);
+    uint64_t* empty = full + TF_MAX_STAGES;
+    uint64_t* tfull = empty + TF_MAX_STAGES;     // accumulator buffer ready for the epilogue
+    uint64_t* tempty = tfull + 2;                // accumulator buffer drained
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nrows = v * vp;                                   // flattened (b,c') rows
+    const int per_job = mtiles * ntiles;
+    const long long nitems = (long long)njobs * per_job;
+    const int kst_v = (v + 7) >> 3, kst_o = (o + 7) >> 3;       // 8-wide k-steps per segment
+    const int nch_v = (v + TF_BK - 1) / TF_BK, nch_o = (o + TF_BK - 1) / TF_BK;
+    const int nch = 2 * (nch_v + nch_o);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(&tfull[b], 1); mbar_init(&tempty[b], 8); }
+        fence_barrier_init();
+    }
+    if (warp == 2) { tmem_alloc(tmem_slot, TF_TMEM_COLS); tmem_relinquish(); }
+    tc_fence_before_sync();
+    __syncthreads();
+    tc_fence_after_sync();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp < 4) reg_dealloc<72>();
+    if (warp == 0) {
+        // ------------------------------------------------------------------------------------ TMA producer
+        if (lane == 0) {
+            for (int h = 0; h < 2; ++h) {
+                tma_prefetch_desc(&maps.xk[h]); tma_prefetch_desc(&maps.xkt[h]); tma_prefetch_desc(&maps.t2k[h]);
+                tma_prefetch_desc(&maps.t2kt[h]); tma_prefetch_desc(&maps.t2a[h]); tma_prefetch_desc(&maps.ota[h]);
+            }
+            uint32_t it = 0;
+            for (long long w = blockIdx.x; w < nitems; w += gridDim.x) {
+                const int jb = (int)(w / per_job), rem = (int)(w % per_job);
+                const int m0 = (rem / ntiles) * TF_BM, a0 = (rem % ntiles) * bn;
+                const GemmJob job = jobs[jb];
+                const int p = job.p, q = job.q, r = job.r;
+                for (int c = 0; c < nch; ++c, ++it) {
+                    const int s = it % stages;
+                    mbar_wait(&empty[s], ((it / stages) & 1) ^ 1);
+                    uint8_t* sM = smem + s * stage_bytes;           // [hi 128 rows][lo 128 rows]
+                    uint8_t* sN = sM + 2 * TF_BM * 128;             // [hi bn rows][lo bn rows]
+                    mbar_arrive_expect_tx(&full[s], stage_bytes);
+                    const CUtensorMap *mm, *nm;
+                    int kk, mz, nz;
+                    if (c < nch_v)                     { kk = c * TF_BK;                       mm = maps.xk;   mz = r; nm = maps.t2a; nz = p * o + q; }
+                    else if (c < 2 * nch_v)            { kk = (c - nch_v) * TF_BK;             mm = maps.xkt;  mz = q; nm = maps.t2a; nz = p * o + r; }
+                    else if (c < 2 * nch_v + nch_o)    { kk = (c - 2 * nch_v) * TF_BK;         mm = maps.t2k;  mz = q; nm = maps.ota; nz = r * o + p; }
+                    else                               { kk = (c - 2 * nch_v - nch_o) * TF_BK; mm = maps.t2kt; mz = r; nm = maps.ota; nz = q * o + p; }
+                    tma_load_3d(sM, &mm[0], &full[s], kk, m0, mz);
+                    tma_load_3d(sM + TF_BM * 128, &mm[1], &full[s], kk, m0, mz);
+                    tma_load_3d(sN, &nm[0], &full[s], kk, a0, nz);
+                    tma_load_3d(sN + bn * 128, &nm[1], &full[s], kk, a0, nz);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ------------------------------------------------------------------------------------ MMA issuer
+        if (lane == 0) {
+            const uint32_t idesc = umma_idesc_tf32_m128((uint32_t)bn);
+            const uint32_t smem_base = smem_u32(smem);
+            uint32_t it = 0, chain = 0;
+            for (long long w = blockIdx.x; w < nitems; w += gridDim.x) {
+                for (int c = 0; c < nch; ++c, ++it) {
+                    const int s = it % stages;
+                    int left;   // k-steps of this chunk that carry data
+                    if (c < nch_v) left = kst_v - c * 4;
+                    else if (c < 2 * nch_v) left = kst_v - (c - nch_v) * 4;
+                    else if (c < 2 * nch_v + nch_o) left = kst_o - (c - 2 * nch_v) * 4;
+                    else left = kst_o - (c - 2 * nch_v - nch_o) * 4;
+                    const int nk = left < 4 ? left : 4;
+                    const uint32_t buf = chain & 1;
+                    const bool first = (c % TF_CHAIN) == 0, last = (c % TF_CHAIN) == TF_CHAIN - 1 || c == nch - 1;
+                    if (first) {
+                        mbar_wait(&tempty[buf], ((chain >> 1) & 1) ^ 1);
+                        tc_fence_after_sync();
+                    }
+                    mbar_wait(&full[s], (it / stages) & 1);
+                    tc_fence_after_sync();
+                    const uint32_t tacc = tmem_base + buf * 256;
+                    const uint32_t sM = smem_base + s * stage_bytes;
+                    const uint32_t sN = sM + 2 * TF_BM * 128;
+                    const uint64_t mh = umma_desc_sw128(sM), ml = umma_desc_sw128(sM + TF_BM * 128);
+                    const uint64_t nh = umma_desc_sw128(sN), nl = umma_desc_sw128(sN + bn * 128);
+                    uint32_t acc = first ? 0u : 1u;
+                    for (int k = 0; k < nk; ++k) {                   // small terms first
+                        const uint64_t adv = (uint64_t)(k * 2);      // 32 bytes per k-step, in 16-byte units
+                        umma_tf32(tacc, ml + adv, nh + adv, idesc, acc);      // lo*hi
+                        acc = 1;
+                        umma_tf32(tacc, mh + adv, nl + adv, idesc, 1);        // hi*lo
+                    }
+                    for (int k = 0; k < nk; ++k) {
+                        const uint64_t adv = (uint64_t)(k * 2);
+                        umma_tf32(tacc, mh + adv, nh + adv, idesc, 1);        // hi*hi
+                    }
+                    umma_commit(&empty[s]);       // smem slot free once these MMAs have read it
+                    if (last) { umma_commit(&tfull[buf]); ++chain; }   // chain complete
+                }
+            }
+        }
+    } else if (warp >= 4) {
+        // ------------------------------------------------------------------------------------ accumulator warps
+        reg_alloc<208>();   // 128*72 + 256*208 <= 64K registers
+        const int wq = warp & 3;                 // TMEM lane quarter this warp may read
+        const int half = (warp - 4) >> 2;        // columns [128*half, 128*half + 128)
+        const int nchain = (nch + TF_CHAIN - 1) / TF_CHAIN;
+        const bool active = half * 128 < bn;
+        uint32_t chain = 0;
+        for (long long w = blockIdx.x; w < nitems; w += gridDim.x) {
+            const int jb = (int)(w / per_job), rem = (int)(w % per_job);
+            const int m0 = (rem / ntiles) * TF_BM, a0 = (rem % ntiles) * bn;
+            float acc[128];
+#pragma unroll
+            for (int j = 0; j < 128; ++j) acc[j] = 0.0f;
+            for (int ch = 0; ch < nchain; ++ch, ++chain) {
+                const uint32_t buf = chain & 1;
+                mbar_wait(&tfull[buf], (chain >> 1) & 1);
+                tc_fence_after_sync();
+                if (active) {
+                    const uint32_t taddr = tmem_base + buf * 256 + half * 128 + ((uint32_t)(wq * 32) << 16);
+#pragma unroll
+                    for (int c0 = 0; c0 < 128; c0 += 16) {
+                        uint32_t rg[16];
+                        tmem_ld_32x32b_x16(taddr + c0, rg);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) acc[c0 + j] = __fadd_rn(acc[c0 + j], __uint_as_float(rg[j]));
+                    }
+                }
+                tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&tempty[buf]);
+            }
+            const int row = m0 + wq * 32 + lane;
+            if (active && row < nrows) {
+                float* __restrict__ out = static_cast<float*>(jobs[jb].out);
+#pragma unroll
+                for (int j = 0; j < 128; ++j) {
+                    const int cl = half * 128 + j;
+                    if (cl < bn && a0 + cl < v) out[(size_t)(a0 + cl) * nrows + row] = acc[j];
+                }
+            }
+        }
+    }
+    tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 2) { tc_fence_after_sync(); tmem_dealloc(tmem_base, TF_TMEM_COLS); }
+}
+
+}  // namespace tb

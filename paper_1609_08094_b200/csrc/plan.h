@@ -55,12 +55,16 @@ enum GemmCfgId { CFG_M120_N128 = 0, CFG_M80_N192 = 1, CFG_M40_N256 = 2 };
 
 struct Plan {
     int o = 0, v = 0, vp = 0, op = 0, prec = 0;
-    int cfg = 0, BM = 0, BN = 0, mtiles = 0, ntiles = 0;
+    int vk = 0, ok = 0;         // mixed path: K pitches of the K-major FP32 operands (v, o rounded up to 4)
+    int cfg = 0, BM = 0, BN = 0, mtiles = 0, ntiles = 0;      // FP64 contraction tiles
+    int tf_bn = 0, tf_ntiles = 0, tf_mtiles = 0;              // mixed contraction tiles: 128 (b,c) rows x tf_bn a-columns
     int nb = 0;                 // triplets per batch
     long long T = 0;            // restricted triplets
     int norb = 0;
     size_t esz = 8;             // bytes per stored operand / U element
     size_t n_x = 0, n_ot = 0, n_t2 = 0, n_u = 0;   // elements of one X (or XT), Ot, T2, one U buffer
+    size_t n_t2k = 0;                              // mixed: elements of T2K (or T2KT)
+    size_t off_t2k = 0, off_t2kt = 0, off_t2klo = 0, off_t2ktlo = 0;
     // workspace offsets (bytes)
     size_t off_x = 0, off_xt = 0, off_ot = 0, off_t2 = 0, off_xlo = 0, off_xtlo = 0, off_otlo = 0, off_t2lo = 0;
     size_t off_u = 0, off_part = 0, off_etrip = 0, off_result = 0, off_gjobs = 0, off_rjobs = 0, off_fjobs = 0,
@@ -100,9 +104,23 @@ inline bool make_plan(int o, int v, int prec, Plan& P) {
     P.n_ot = (size_t)o * o * v * P.op;
     P.n_t2 = (size_t)o * o * v * P.vp;
     P.n_u = (size_t)v * v * P.vp;
-    // batch: enough CTAs for >= 40 waves of 148 SMs, U buffers capped at 12 GiB, at least one triplet
-    const long long ctas_per_triplet = 3LL * P.mtiles * P.ntiles;
-    long long nb = (40LL * kNumSM + ctas_per_triplet - 1) / ctas_per_triplet;
+    long long ctas_per_triplet = 3LL * P.mtiles * P.ntiles;
+    long long waves = 40;
+    if (prec == 1) {   // K-major FP32 operands, transposed tiles (gemm_tf32.cuh)
+        P.vk = (v + 3) & ~3;
+        P.ok = (o + 3) & ~3;
+        P.tf_ntiles = (v + 255) / 256;
+        P.tf_bn = (((v + P.tf_ntiles - 1) / P.tf_ntiles) + 15) & ~15;
+        P.tf_mtiles = (int)((N + 127) / 128);
+        P.n_x = (size_t)o * v * P.vp * P.vk;
+        P.n_t2 = (size_t)o * o * v * P.vk;
+        P.n_ot = (size_t)o * o * v * P.ok;
+        P.n_t2k = (size_t)o * v * P.vp * P.ok;
+        ctas_per_triplet = 3LL * P.tf_mtiles * P.tf_ntiles;
+        waves = 60;
+    }
+    // batch: enough CTAs for >= `waves` waves of 148 SMs, U buffers capped at 12 GiB, at least one triplet
+    long long nb = (waves * kNumSM + ctas_per_triplet - 1) / ctas_per_triplet;
     const long long cap = (long long)((12ULL << 30) / (3 * P.n_u * P.esz));
     if (nb > cap) nb = cap;
     if (nb > P.T) nb = P.T;
@@ -121,6 +139,10 @@ inline bool make_plan(int o, int v, int prec, Plan& P) {
         P.off_xtlo = take(P.n_x * P.esz);
         P.off_otlo = take(P.n_ot * P.esz);
         P.off_t2lo = take(P.n_t2 * P.esz);
+        P.off_t2k = take(P.n_t2k * P.esz);
+        P.off_t2kt = take(P.n_t2k * P.esz);
+        P.off_t2klo = take(P.n_t2k * P.esz);
+        P.off_t2ktlo = take(P.n_t2k * P.esz);
     }
     P.off_u = take((size_t)P.nb * 3 * P.n_u * P.esz);
     P.off_part = take((size_t)P.nb * P.norb * 16);

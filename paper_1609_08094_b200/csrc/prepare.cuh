@@ -96,4 +96,75 @@ __global__ void pack_t2_kernel(const double* __restrict__ t2, size_t rows, int v
     }
 }
 
+// ------------------------------------------------------------------------------------------------ mixed path
+// K-major FP32 operands of gemm_tf32.cuh, each as a hi/lo pair (Splitter<float>):
+//   XK  [r][b][c][d] = vvvo[d][b][c][r] = (db|cr)      (c: vp rows per b, d-pitch vk = v rounded up to 4)
+//   XKT [r][b][c][d] = XK[r][c][b][d]
+//   T2K [q][b][c][l] = t2[q][l][b][c]                  (l-pitch ok = o rounded up to 4)
+//   T2KT[r][b][c][l] = t2[l][r][b][c] = t2[r][l][c][b]
+//   T2A = pack_t2_kernel with pitch vk, OtA = pack_ot_kernel with pitch ok.
+// Pads are zeroed by the caller (cudaMemsetAsync) when any exists.
+
+// vvvo viewed as [d][s = (b,c,r) flat, v*v*o]: one CTA moves a (32 d) x (PKX_SPAN s) brick through smem and writes
+// rows of 32 consecutive d (128 bytes).
+constexpr int PKX_SPAN = 256;
+constexpr int PKX_PITCH = PKX_SPAN + 1;
+constexpr int PKX_SMEM = 32 * PKX_PITCH * 8;
+__global__ void __launch_bounds__(256)
+pack_xk_kernel(const double* __restrict__ vvvo, int v, int vp, int vk, int o, float* __restrict__ XK,
+               float* __restrict__ XKlo, float* __restrict__ XKT, float* __restrict__ XKTlo) {
+    extern __shared__ double tile[];                 // [32][PKX_PITCH]
+    const int d0 = blockIdx.y * 32;
+    const size_t S = (size_t)v * v * o;
+    const size_t s0 = (size_t)blockIdx.x * PKX_SPAN;
+    const int cnt = (int)min((size_t)PKX_SPAN, S - s0);
+    for (int e = threadIdx.x; e < 32 * cnt; e += 256) {
+        const int dd = e / cnt, s = e % cnt;
+        if (d0 + dd < v) tile[dd * PKX_PITCH + s] = vvvo[(size_t)(d0 + dd) * S + s0 + s];
+    }
+    __syncthreads();
+    const size_t plane = (size_t)v * vp * vk;        // one r-slice
+    for (int e = threadIdx.x; e < 32 * cnt; e += 256) {
+        const int dd = e & 31, s = e >> 5;
+        if (d0 + dd >= v) continue;
+        const size_t sg = s0 + s;
+        const int r = (int)(sg % o);
+        const size_t bc = sg / o;
+        const int b = (int)(bc / v), c = (int)(bc % v);
+        const double x = tile[dd * PKX_PITCH + s];
+        const float h = to_tf32_rn((float)x);
+        const float l = to_tf32_rn((float)(x - (double)h));
+        const size_t i1 = (size_t)r * plane + ((size_t)b * vp + c) * vk + d0 + dd;
+        const size_t i2 = (size_t)r * plane + ((size_t)c * vp + b) * vk + d0 + dd;
+        XK[i1] = h; XKlo[i1] = l;
+        XKT[i2] = h; XKTlo[i2] = l;
+    }
+}
+
+// blockIdx.x = q*v + x (x = b for T2K, x = c for T2KT), blockIdx.y = chunk of 64 along the contiguous source index y,
+// blockIdx.z = chunk of 64 along l.
+__global__ void __launch_bounds__(256)
+pack_t2k_kernel(const double* __restrict__ t2, int v, int vp, int o, int ok, float* __restrict__ T2K,
+                float* __restrict__ T2Klo, float* __restrict__ T2KT, float* __restrict__ T2KTlo) {
+    __shared__ double tile[64][65];
+    const int q = blockIdx.x / v, x = blockIdx.x % v;
+    const int y0 = blockIdx.y * 64, l0 = blockIdx.z * 64;
+    const int ny = min(64, v - y0), nl = min(64, o - l0);
+    for (int e = threadIdx.x; e < nl * ny; e += 256) {
+        const int l = e / ny, yy = e % ny;
+        tile[l][yy] = t2[(((size_t)q * o + l0 + l) * v + x) * v + y0 + yy];      // t2[q][l][x][y]
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < nl * ny; e += 256) {
+        const int l = e % nl, yy = e / nl;
+        const double val = tile[l][yy];
+        const float h = to_tf32_rn((float)val);
+        const float lo = to_tf32_rn((float)(val - (double)h));
+        const size_t i1 = (((size_t)q * v + x) * vp + (y0 + yy)) * ok + l0 + l;   // T2K [q][b=x][c=y][l]
+        const size_t i2 = (((size_t)q * v + (y0 + yy)) * vp + x) * ok + l0 + l;   // T2KT[q][b=y][c=x][l] = t2[q][l][x][y]
+        T2K[i1] = h; T2Klo[i1] = lo;
+        T2KT[i2] = h; T2KTlo[i2] = lo;
+    }
+}
+
 }  // namespace tb

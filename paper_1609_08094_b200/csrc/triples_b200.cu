@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "gemm_f64.cuh"
+#include "gemm_tf32.cuh"
 #include "plan.h"
 #include "prepare.cuh"
 #include "reduce.cuh"
@@ -130,6 +131,12 @@ int launch_gemm_f64(const GemmMaps& maps, const GemmJob* jobs, int njobs, const 
 struct Operands {   // device pointers of the repacked operands (workspace) for one precision
     void *x, *xt, *ot, *t2;
     void *xlo, *xtlo, *otlo, *t2lo;
+    void *t2k, *t2kt, *t2klo, *t2ktlo;   // mixed path only
+};
+
+struct Maps {   // tensor maps of the contraction kernel of the plan's precision
+    GemmMaps f64;
+    Tf32Maps tf32;
 };
 
 int build_maps_f64(const Plan& P, const Operands& op, GemmMaps* maps) {
@@ -145,19 +152,102 @@ int build_maps_f64(const Plan& P, const Operands& op, GemmMaps* maps) {
     return TRIPLES_OK;
 }
 
-int launch_gemm(const Plan& P, const GemmMaps& maps, const GemmJob* jobs, int njobs, cudaStream_t st) {
-    if (P.prec != TRIPLES_FP64) return fail(TRIPLES_EINVAL, "mixed-precision contraction path is not built in this version");
+int build_maps_tf32(const Plan& P, const Operands& op, Tf32Maps* maps) {
+    const uint64_t o = P.o, v = P.v, vk = P.vk, ok = P.ok, NR = (uint64_t)P.v * P.vp;
+    const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const void* xk[2] = {op.x, op.xlo};
+    const void* xkt[2] = {op.xt, op.xtlo};
+    const void* t2k[2] = {op.t2k, op.t2klo};
+    const void* t2kt[2] = {op.t2kt, op.t2ktlo};
+    const void* t2a[2] = {op.t2, op.t2lo};
+    const void* ota[2] = {op.ot, op.otlo};
+    int rc;
+    for (int h = 0; h < 2; ++h) {
+        if ((rc = make_map3(&maps->xk[h], dt, 4, xk[h], v, NR, o, vk, NR * vk, TF_BK, TF_BM, 1))) return rc;
+        if ((rc = make_map3(&maps->xkt[h], dt, 4, xkt[h], v, NR, o, vk, NR * vk, TF_BK, TF_BM, 1))) return rc;
+        if ((rc = make_map3(&maps->t2k[h], dt, 4, t2k[h], o, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
+        if ((rc = make_map3(&maps->t2kt[h], dt, 4, t2kt[h], o, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
+        if ((rc = make_map3(&maps->t2a[h], dt, 4, t2a[h], v, v, o * o, vk, v * vk, TF_BK, P.tf_bn, 1))) return rc;
+        if ((rc = make_map3(&maps->ota[h], dt, 4, ota[h], o, v, o * o, ok, v * ok, TF_BK, P.tf_bn, 1))) return rc;
+    }
+    return TRIPLES_OK;
+}
+
+int build_maps(const Plan& P, const Operands& op, Maps* maps) {
+    return P.prec == TRIPLES_FP64 ? build_maps_f64(P, op, &maps->f64) : build_maps_tf32(P, op, &maps->tf32);
+}
+
+int launch_gemm_tf32(const Tf32Maps& maps, const GemmJob* jobs, int njobs, const Plan& P, cudaStream_t st) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        CU_TRY(cudaFuncSetAttribute(gemm_tf32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TF_SMEM_LIMIT));
+        attr_set = true;
+    }
+    const long long items = (long long)njobs * P.tf_mtiles * P.tf_ntiles;
+    if (items == 0) return TRIPLES_OK;
+    const int grid = (int)std::min<long long>(items, kNumSM);
+    gemm_tf32_kernel<<<grid, TF_THREADS, tf32_smem_bytes(P.tf_bn), st>>>(maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles,
+                                                                        P.tf_ntiles, P.tf_bn);
+    CU_TRY(cudaGetLastError());
+    ++g_launches;
+    return TRIPLES_OK;
+}
+
+int launch_gemm(const Plan& P, const Maps& maps, const GemmJob* jobs, int njobs, cudaStream_t st) {
+    if (P.prec == TRIPLES_MIXED) return launch_gemm_tf32(maps.tf32, jobs, njobs, P, st);
     switch (P.cfg) {
-        case CFG_M120_N128: return launch_gemm_f64<3, 4, 4, 4>(maps, jobs, njobs, P, st);
-        case CFG_M80_N192: return launch_gemm_f64<2, 4, 6, 4>(maps, jobs, njobs, P, st);
-        default: return launch_gemm_f64<1, 8, 4, 4>(maps, jobs, njobs, P, st);
+        case CFG_M120_N128: return launch_gemm_f64<3, 4, 4, 4>(maps.f64, jobs, njobs, P, st);
+        case CFG_M80_N192: return launch_gemm_f64<2, 4, 6, 4>(maps.f64, jobs, njobs, P, st);
+        default: return launch_gemm_f64<1, 8, 4, 4>(maps.f64, jobs, njobs, P, st);
     }
 }
 
 // ------------------------------------------------------------------------------------------ prepare (S0)
+// Mixed path: K-major FP32 hi/lo operands of gemm_tf32.cuh.
+int run_prepare_mixed(const Plan& P, const double* t2, const double* vvvo, const double* ovoo, const Operands& op,
+                      cudaStream_t st) {
+    const int o = P.o, v = P.v;
+    if (P.vp != v || P.vk != v) {
+        for (void* ptr : {op.x, op.xlo, op.xt, op.xtlo}) CU_TRY(cudaMemsetAsync(ptr, 0, P.n_x * 4, st));
+        for (void* ptr : {op.t2, op.t2lo}) CU_TRY(cudaMemsetAsync(ptr, 0, P.n_t2 * 4, st));
+    }
+    if (P.vp != v || P.ok != o)
+        for (void* ptr : {op.t2k, op.t2klo, op.t2kt, op.t2ktlo}) CU_TRY(cudaMemsetAsync(ptr, 0, P.n_t2k * 4, st));
+    if (P.ok != o)
+        for (void* ptr : {op.ot, op.otlo}) CU_TRY(cudaMemsetAsync(ptr, 0, P.n_ot * 4, st));
+    {
+        static bool attr_set = false;
+        if (!attr_set) {
+            CU_TRY(cudaFuncSetAttribute(pack_xk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PKX_SMEM));
+            attr_set = true;
+        }
+        const size_t S = (size_t)v * v * o;
+        dim3 grid((unsigned)((S + PKX_SPAN - 1) / PKX_SPAN), (v + 31) / 32);
+        pack_xk_kernel<<<grid, 256, PKX_SMEM, st>>>(vvvo, v, P.vp, P.vk, o, (float*)op.x, (float*)op.xlo, (float*)op.xt,
+                                                    (float*)op.xtlo);
+        CU_TRY(cudaGetLastError());
+        ++g_launches;
+    }
+    {
+        dim3 grid(o * v, (v + 63) / 64, (o + 63) / 64);
+        pack_t2k_kernel<<<grid, 256, 0, st>>>(t2, v, P.vp, o, P.ok, (float*)op.t2k, (float*)op.t2klo, (float*)op.t2kt,
+                                              (float*)op.t2ktlo);
+        CU_TRY(cudaGetLastError());
+        ++g_launches;
+    }
+    pack_ot_kernel<float><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.ok, (float*)op.ot, (float*)op.otlo);
+    CU_TRY(cudaGetLastError());
+    ++g_launches;
+    pack_t2_kernel<float><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vk, (float*)op.t2, (float*)op.t2lo);
+    CU_TRY(cudaGetLastError());
+    ++g_launches;
+    return TRIPLES_OK;
+}
+
 template <typename TO>
 int run_prepare(const Plan& P, const double* t2, const double* vvvo, const double* ovoo, const Operands& op,
                 cudaStream_t st) {
+    if (P.prec == TRIPLES_MIXED) return run_prepare_mixed(P, t2, vvvo, ovoo, op, st);
     const int o = P.o, v = P.v;
     const bool split = P.prec == TRIPLES_MIXED;
     if (P.vp != v) {   // zero the pad columns
@@ -215,6 +305,7 @@ Operands carve_operands(const Plan& P, uint8_t* ws) {
     op.x = ws + P.off_x; op.xt = ws + P.off_xt; op.ot = ws + P.off_ot; op.t2 = ws + P.off_t2;
     if (P.prec == TRIPLES_MIXED) {
         op.xlo = ws + P.off_xlo; op.xtlo = ws + P.off_xtlo; op.otlo = ws + P.off_otlo; op.t2lo = ws + P.off_t2lo;
+        op.t2k = ws + P.off_t2k; op.t2kt = ws + P.off_t2kt; op.t2klo = ws + P.off_t2klo; op.t2ktlo = ws + P.off_t2ktlo;
     }
     return op;
 }
@@ -242,12 +333,8 @@ int run_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, c
     if (int rc = run_prepare<TS>(P, in.t2, in.vvvo, in.ovoo, op, st)) return rc;
     if (prof) CU_TRY(cudaEventRecord(ev_p1, st));
 
-    GemmMaps maps;
-    if (P.prec == TRIPLES_FP64) {
-        if (int rc = build_maps_f64(P, op, &maps)) return rc;
-    } else {
-        return fail(TRIPLES_EINVAL, "mixed-precision contraction path is not built in this version");
-    }
+    Maps maps;
+    if (int rc = build_maps(P, op, &maps)) return rc;
 
     // ---- job tables for every batch, uploaded once
     std::vector<Orbit> orbits;
@@ -500,21 +587,26 @@ int triples_w_block(int nocc, int nvirt, const double* t2, const double* vvvo, c
         if (misaligned(ptrs[n])) return fail(TRIPLES_EINVAL, "input pointer #%d is not 16-byte aligned", n);
     if (workspace_bytes < P.total)
         return fail(TRIPLES_EWORKSPACE, "workspace too small: %zu bytes given, %zu needed", workspace_bytes, P.total);
-    if (precision != TRIPLES_FP64) return fail(TRIPLES_EINVAL, "mixed-precision contraction path is not built in this version");
     if (int rc = check_device()) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     uint8_t* ws = static_cast<uint8_t*>(workspace);
     Operands op = carve_operands(P, ws);
     g_launches = 0;
     if (int rc = run_prepare<double>(P, t2, vvvo, ovoo, op, st)) return rc;
-    GemmMaps maps;
-    if (int rc = build_maps_f64(P, op, &maps)) return rc;
-    double* ubase = reinterpret_cast<double*>(ws + P.off_u);
-    GemmJob gj[3] = {{i, j, k, 0, ubase}, {j, i, k, 0, ubase + P.n_u}, {k, i, j, 0, ubase + 2 * P.n_u}};
+    Maps maps;
+    if (int rc = build_maps(P, op, &maps)) return rc;
+    uint8_t* ubase = ws + P.off_u;
+    const size_t ub = P.n_u * P.esz;   // bytes of one U buffer
+    GemmJob gj[3] = {{i, j, k, 0, ubase}, {j, i, k, 0, ubase + ub}, {k, i, j, 0, ubase + 2 * ub}};
     GemmJob* d_gj = reinterpret_cast<GemmJob*>(ws + P.off_gjobs);
     CU_TRY(cudaMemcpyAsync(d_gj, gj, sizeof gj, cudaMemcpyHostToDevice, st));
     if (int rc = launch_gemm(P, maps, d_gj, 3, st)) return rc;
-    assemble_w_kernel<double><<<kNumSM * 4, 256, 0, st>>>(ubase, ubase + P.n_u, ubase + 2 * P.n_u, nvirt, P.vp, W_out);
+    if (precision == TRIPLES_FP64)
+        assemble_w_kernel<double><<<kNumSM * 4, 256, 0, st>>>((const double*)ubase, (const double*)(ubase + ub),
+                                                               (const double*)(ubase + 2 * ub), nvirt, P.vp, W_out);
+    else
+        assemble_w_kernel<float><<<kNumSM * 4, 256, 0, st>>>((const float*)ubase, (const float*)(ubase + ub),
+                                                              (const float*)(ubase + 2 * ub), nvirt, P.vp, W_out);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     CU_TRY(cudaStreamSynchronize(st));
