@@ -19,12 +19,14 @@
 // (rho) and a column permutation of its N index (nu); see DESIGN.md "contraction kernel".
 #pragma once
 #include "ptx.cuh"
+#include "ulayout.cuh"
 
 namespace tb {
 
 struct GemmJob {
     int p, q, r, pad;
-    void* out;  // [v][N] row-major, N = v*vp
+    void* out;   // G(p,q,r)[a][b][c] in the blocked layout of ulayout.cuh: slot base + u * UBLK
+    void* out2;  // second destination (or null): a triplet with i=j or j=k uses the same G twice
 };
 
 struct alignas(64) GemmMaps {
@@ -176,18 +178,24 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
         if (lane == 0) mbar_arrive(&empty[s]);
     }
 
-    // ---------------------------------------------------------------- epilogue: natural-order store
+    // ---------------------------------------------------------------- epilogue: blocked + swizzled store (ulayout.cuh)
+    // column n = b*vp + c (c even): the pair (c, c+1) is one 16-byte word of the 8x8x8 block of (row, b, c)
     double* __restrict__ out = static_cast<double*>(job.out);
+    double* __restrict__ out2 = static_cast<double*>(job.out2);
+    const int nt = u_tiles(v);
 #pragma unroll
-    for (int i = 0; i < MT; ++i) {
-        const int row = m0 + wm * MT * 8 + i * 8 + rg;
-        if (row < v) {
+    for (int j = 0; j < NT; ++j) {
+        const int col = n0 + (wn * (NT / 2) + (j >> 1)) * 16 + (j & 1) * 4 + nu_col(2 * t);
+        const int bb = col / vp, cc = col - bb * vp;
+        if (col < N && cc < v) {
+            const size_t cb = ((size_t)(bb >> 3) * nt + (cc >> 3)) * UCHUNK;
 #pragma unroll
-            for (int j = 0; j < NT; ++j) {
-                const int col = n0 + (wn * (NT / 2) + (j >> 1)) * 16 + (j & 1) * 4 + nu_col(2 * t);
-                if (col < N) {
-                    double2 val = make_double2(acc[i][j][0], acc[i][j][1]);
-                    *reinterpret_cast<double2*>(out + (size_t)row * N + col) = val;
+            for (int i = 0; i < MT; ++i) {
+                const int row = m0 + wm * MT * 8 + i * 8 + rg;
+                if (row < v) {
+                    const size_t off = (size_t)(row >> 3) * nt * nt * UCHUNK + cb + u_swz<8>(row & 7, bb & 7, cc & 7);
+                    *reinterpret_cast<double2*>(out + off) = make_double2(acc[i][j][0], acc[i][j][1]);
+                    if (out2) *reinterpret_cast<double2*>(out2 + off) = make_double2(acc[i][j][0], acc[i][j][1]);
                 }
             }
         }

@@ -30,6 +30,7 @@
 #pragma once
 #include "gemm_f64.cuh"   // GemmJob
 #include "ptx.cuh"
+#include "ulayout.cuh"
 
 namespace tb {
 
@@ -202,13 +203,23 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&tempty[buf]);
             }
+            // blocked + swizzled store (ulayout.cuh): this thread owns (b,c) = row, the columns are a
             const int row = m0 + wq * 32 + lane;
-            if (active && row < nrows) {
+            const int bb = row / vp, cc = row - bb * vp;
+            if (active && row < nrows && cc < v) {
                 float* __restrict__ out = static_cast<float*>(jobs[jb].out);
+                float* __restrict__ out2 = static_cast<float*>(jobs[jb].out2);
+                const int nt = u_tiles(v);
+                const size_t cb = ((size_t)(bb >> 3) * nt + (cc >> 3)) * UCHUNK + u_swz<4>(0, bb & 7, cc & 7);
+                const size_t astride = (size_t)nt * nt * UCHUNK;   // one a-tile
 #pragma unroll
                 for (int j = 0; j < 128; ++j) {
-                    const int cl = half * 128 + j;
-                    if (cl < bn && a0 + cl < v) out[(size_t)(a0 + cl) * nrows + row] = acc[j];
+                    const int cl = half * 128 + j;                 // a0 is a multiple of 16: (a0 + cl) & 7 = j & 7
+                    if (cl < bn && a0 + cl < v) {
+                        const size_t off = (size_t)((a0 + cl) >> 3) * astride + (cb ^ (size_t)u_swz<4>(j & 7, 0, 0));
+                        out[off] = acc[j];
+                        if (out2) out2[off] = acc[j];
+                    }
                 }
             }
         }

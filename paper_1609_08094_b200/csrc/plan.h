@@ -10,6 +10,7 @@ namespace tb {
 constexpr int kMaxVirt = 2040;   // tile indices of the 8-wide reduction tiles fit a byte
 constexpr int kMaxOcc = 1024;
 constexpr int kNumSM = 148;
+constexpr int kRedWarps = 8;     // consumer warps of the fused reduction: one partial per (triplet, orbit, warp)
 
 struct Triplet { int i, j, k; long long index; };   // index = position in the i<=j<=k enumeration
 
@@ -60,7 +61,10 @@ struct Plan {
     int tf_bn = 0, tf_ntiles = 0, tf_mtiles = 0;              // mixed contraction tiles: 128 (b,c) rows x tf_bn a-columns
     int nb = 0;                 // triplets per batch
     long long T = 0;            // restricted triplets
-    int norb = 0;
+    int norb = 0, nt = 0;       // tile orbits, 8-wide tiles per virtual axis
+    int red_gx = 0;             // CTA columns of the fused reduction (orbit stride), fixed by v
+    size_t n_side = 0;          // doubles of one triplet's side buffer (reduce.cuh)
+    size_t off_side = 0;
     size_t esz = 8;             // bytes per stored operand / U element
     size_t n_x = 0, n_ot = 0, n_t2 = 0, n_u = 0;   // elements of one X (or XT), Ot, T2, one U buffer
     size_t n_t2k = 0;                              // mixed: elements of T2K (or T2KT)
@@ -103,7 +107,9 @@ inline bool make_plan(int o, int v, int prec, Plan& P) {
     P.n_x = (size_t)o * v * v * P.vp;
     P.n_ot = (size_t)o * o * v * P.op;
     P.n_t2 = (size_t)o * o * v * P.vp;
-    P.n_u = (size_t)v * v * P.vp;
+    P.nt = num_red_tiles(v);
+    P.n_u = (size_t)P.nt * P.nt * P.nt * 512;          // blocked layout of ulayout.cuh
+    P.n_side = (size_t)P.nt * P.nt * 448;             // tile-pair records of reduce.cuh
     long long ctas_per_triplet = 3LL * P.mtiles * P.ntiles;
     long long waves = 40;
     if (prec == 1) {   // K-major FP32 operands, transposed tiles (gemm_tf32.cuh)
@@ -145,7 +151,9 @@ inline bool make_plan(int o, int v, int prec, Plan& P) {
         P.off_t2ktlo = take(P.n_t2k * P.esz);
     }
     P.off_u = take((size_t)P.nb * 3 * P.n_u * P.esz);
-    P.off_part = take((size_t)P.nb * P.norb * 16);
+    P.red_gx = P.norb < kNumSM ? P.norb : kNumSM;
+    P.off_part = take((size_t)P.nb * P.red_gx * kRedWarps * 16);
+    P.off_side = take((size_t)P.nb * P.n_side * 8);
     P.off_etrip = take((size_t)P.T * 3 * 8);
     P.off_result = take(256);
     P.off_gjobs = take((size_t)P.T * 3 * 32);

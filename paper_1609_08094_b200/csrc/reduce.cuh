@@ -1,176 +1,317 @@
 // reduce.cuh -- fused permutation-accumulate + V assembly + denominator + energy contraction (S4-S7),
 // the per-triplet finalize (S8a) and the deterministic total (S8b).
 //
-// Per triplet (i<=j<=k) the contraction kernel left three natural-order buffers
-//   U1 = G(i,j,k)[a][b][c],  U2 = G(j,i,k)[b][a][c],  U3 = G(k,i,j)[c][a][b]      (c-pitch vp)
+// Per triplet (i<=j<=k) the contraction kernel left three buffers in the blocked layout of ulayout.cuh
+//   U1 = G(i,j,k)[a][b][c],  U2 = G(j,i,k)[b][a][c],  U3 = G(k,i,j)[c][a][b]
 // and W^abc = U1[a,b,c] + U2[b,a,c] + U3[c,a,b]            (Eq. (2.2.3)).
 // The energy of the triplet is  e = sum_abc Z[W]^abc (W + Vd)^abc / D^abc  with
 //   Z[W]^abc = 4W^abc + W^bca + W^cab - 2W^acb - 2W^cba - 2W^bac   (symmetrised Eq. (2.2.5); Q4)
 //   Vd^abc   = t1[i,a] (jb|kc) + t1[j,b] (ia|kc) + t1[k,c] (ia|jb)                 (Eq. (2.2.4))
 //   D^abc    = eps_i + eps_j + eps_k - eps_a - eps_b - eps_c                       (L92, L65; Q1)
 //
-// One CTA owns one *tile orbit* {A<=B<=C} of 8x8x8 blocks of the virtual cube: it stages W on the six
-// permuted blocks in shared memory (every U element of the orbit is read from HBM once), then every thread
-// walks index triples (a in A, b in B, c in C) and adds the contribution of all six permutations of (a,b,c):
-//   w_pi = W at the six permutations;  E = w_abc + w_bca + w_cab (even),  O = w_acb + w_bac + w_cba (odd)
-//   sum_pi Z_pi w_pi  = 3 sum w_pi^2 + (E-O)^2 - 2 E O
-//   sum_pi Z_pi vd_pi = sum_pi vd_pi (3 w_pi + [same-parity sum] - 2 [other-parity sum])
-// with one division per index triple (D is symmetric in abc).  Orbits with coinciding tiles visit every element
-// `sym` in {2,6} times and are scaled by 1/sym.
+// Work item = one triplet x one *tile orbit* {A<=B<=C} of 8x8x8 tiles of the virtual cube (not one output tile:
+// otherwise every U element would be fetched six times).  The kernel is persistent (one CTA per SM) and
+// warp-specialised:
+//   warp 8      producer: per item 9 cp.async.bulk copies into the next stage of a shared-memory ring --
+//               6 chunks of 3 U blocks (one per arrangement of (A,B,C); 12 KiB FP64 / 6 KiB FP32 each, every U
+//               element of the orbit read from HBM exactly once) and 3 records {A,B}, {A,C}, {B,C} of the
+//               per-triplet side buffer (side_pack_kernel): the (ov|ov) tiles of both orders of the pair, three
+//               slices each, plus the t1[i|j|k] / eps_v rows of both tiles.  Few, large copies: the TMA unit
+//               spends ~65 clk per bulk copy whatever its size (measured), 27 small copies per item were TMA-bound;
+//   warps 0-7   consumers: every thread owns two index triples (a, a+4 ; b ; c) of the orbit and adds the
+//               contribution of all six permutations of (a,b,c) at once, reading the staged blocks in place
+//               (the swizzle of ulayout.cuh makes all 18 reads bank-conflict free):
+//                 w_pi = W at the six permutations;  E = w_abc + w_bca + w_cab,  O = w_acb + w_bac + w_cba
+//                 sum_pi Z_pi w_pi  = 3 sum w_pi^2 + (E-O)^2 - 2 E O
+//                 sum_pi Z_pi vd_pi = sum_pi vd_pi (3 w_pi + [same-parity sum] - 2 [other-parity sum])
+//               ONE division per index triple (D is symmetric in abc); a thread keeps a running FP64 sum over
+//               all orbits its CTA visits for the triplet, then warp-shuffle tree ->
+//               partials[triplet][CTA column][warp] (fixed layout, no atomics).
+// Orbits with coinciding tiles visit every element `sym` in {2,6} times and are scaled by 1/sym.
+// blockIdx.x strides over the orbits of a triplet and blockIdx.y over the triplets of the batch, so which orbits
+// are summed together depends on v only: a triplet's energy is bitwise the same in every batch composition.
 #pragma once
 #include <cstdint>
 
+#include "ptx.cuh"
+#include "ulayout.cuh"
+
 namespace tb {
 
-template <typename T>
 struct RedJob {
-    int i, j, k, slot;      // slot: row of `partials` this triplet writes
-    const T* u1;
-    const T* u2;
-    const T* u3;
+    int i, j, k, slot;      // slot: which U / side / partials slot of the batch this triplet uses
+    const void* u;          // the slot's interleaved U1,U2,U3 blocks (ulayout.cuh)
+    const void* pad;
 };
 
-constexpr int RT = 8;             // tile edge
-constexpr int RP1 = 9;            // smem pitch of the fastest index
-constexpr int RP2 = 74;           // smem pitch of the middle index (8*9 + 2)
-constexpr int RBLK = RT * RP2;    // one staged block
-constexpr int RED_THREADS = 256;
+constexpr int RED_CONSUMER_WARPS = 8;
+constexpr int RED_THREADS = (RED_CONSUMER_WARPS + 1) * 32;
+// side record of a tile pair P<=Q (doubles): J[P->Q][s][64], J[Q->P][s][64] (Morton inside a tile; s = slice),
+// then {t1[i], t1[j], t1[k], eps_v}[8] of tile P and of tile Q
+constexpr int RED_REC_DOUBLES = 2 * 192 + 2 * 32;
+constexpr int RED_REC_BYTES = RED_REC_DOUBLES * 8;          // 3584
+constexpr int RED_SIDE_BYTES = 3 * RED_REC_BYTES;           // records {A,B}, {A,C}, {B,C}
+constexpr int RED_H_BYTES = 128;              // per-item header written by the producer (generic stores)
 
-template <typename T> struct Vec2;
-template <> struct Vec2<double> { using type = double2; };
-template <> struct Vec2<float> { using type = float2; };
+// side buffer of one triplet (doubles): rec[P][Q], P <= Q used
+__host__ __device__ constexpr size_t side_doubles(int nt) { return (size_t)nt * nt * RED_REC_DOUBLES; }
 
 template <typename T>
-__global__ void __launch_bounds__(RED_THREADS)
-reduce_kernel(const RedJob<T>* __restrict__ jobs, const uchar4* __restrict__ orbits, int norb, int v, int vp, int o,
-              const double* __restrict__ eps_o, const double* __restrict__ eps_v, const double* __restrict__ t1,
-              const double* __restrict__ ovov, double2* __restrict__ partials) {
-    using V2 = typename Vec2<T>::type;
-    __shared__ double S[6 * RBLK];          // W on the six blocks, S[blk][x][y][z]
-    __shared__ double Js[3][6][RT][RP1];    // (ov|ov) slices on the six ordered tile pairs
-    __shared__ double T1s[3][3][RT];        // t1[i|j|k][tile A|B|C]
-    __shared__ double Ev[3][RT];            // eps_v on tiles A,B,C
-    __shared__ double red[2][RED_THREADS / 32];
+struct RedCfg {
+    static constexpr int ESZ = (int)sizeof(T);
+    static constexpr int BLK_BYTES = UBLK * ESZ;
+    static constexpr int U_BYTES = 18 * BLK_BYTES;
+    static constexpr int S_OFF = U_BYTES;                        // the three side records
+    static constexpr int H_OFF = S_OFF + RED_SIDE_BYTES;
+    static constexpr int TX_BYTES = H_OFF;                       // bytes the bulk copies deliver per item
+    static constexpr int STAGE_BYTES = H_OFF + RED_H_BYTES;
+    static constexpr int STAGES = ESZ == 8 ? 2 : 4;
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8 + 128;
+    static_assert(STAGE_BYTES % 128 == 0, "stages stay 128-byte aligned");
+};
 
-    const int tid = threadIdx.x;
-    const RedJob<T> job = jobs[blockIdx.y];
-    const uchar4 orb = orbits[blockIdx.x];
-    const int tl[3] = {orb.x * RT, orb.y * RT, orb.z * RT};   // first index of tiles A, B, C
-    const size_t pa = (size_t)v * vp;                          // pitch of the slowest index of U
+// arrangement pi of (A,B,C) = (0,1,2): 0:(0,1,2) 1:(0,2,1) 2:(1,0,2) 3:(1,2,0) 4:(2,0,1) 5:(2,1,0)
+__host__ __device__ constexpr int arr_x(int pi) { return pi >> 1; }
+__host__ __device__ constexpr int arr_y(int pi) { return (pi & 1) ? (arr_x(pi) == 2 ? 1 : 2) : (arr_x(pi) == 0 ? 1 : 0); }
+__host__ __device__ constexpr int arr_z(int pi) { return 3 - arr_x(pi) - arr_y(pi); }
+__host__ __device__ constexpr int arr_id(int p0, int p1, int p2) { return 2 * p0 + (p1 > p2 ? 1 : 0); }
 
-    // block pi holds W[x][y][z] with x in tile PX[pi], y in PY[pi], z in PZ[pi]  (0=A, 1=B, 2=C)
-    constexpr int PX[6] = {0, 0, 1, 1, 2, 2};
-    constexpr int PY[6] = {1, 2, 0, 2, 0, 1};
-    constexpr int PZ[6] = {2, 1, 2, 0, 1, 0};
+// launch geometry: blockIdx.x strides over the orbits of a triplet, blockIdx.y over the triplets of the batch.
+// The set of orbits a CTA sums for one triplet depends on v only, never on the batch, so per-triplet energies are
+// bitwise identical whichever batch a triplet is computed in.
+__host__ __device__ constexpr int red_grid_x(int norb, int nsm) { return norb < nsm ? norb : nsm; }
 
-    // ---- issue all global loads of the orbit first (18 vector loads per thread in flight)
-    V2 r1[6], r2[6], r3[6];
-    {
-        const int x = tid >> 5, y = (tid >> 2) & 7, z = (tid & 3) * 2;       // U1/U2: z pairs contiguous
-        const int z3 = tid >> 5, x3 = (tid >> 2) & 7, y3 = (tid & 3) * 2;    // U3:    y pairs contiguous
-#pragma unroll
-        for (int b = 0; b < 6; ++b) {
-            const int X0 = tl[PX[b]], Y0 = tl[PY[b]], Z0 = tl[PZ[b]];
-            V2 zero; zero.x = 0; zero.y = 0;
-            r1[b] = zero; r2[b] = zero; r3[b] = zero;
-            if (X0 + x < v && Y0 + y < v && Z0 + z < v) {
-                r1[b] = *reinterpret_cast<const V2*>(job.u1 + (size_t)(X0 + x) * pa + (size_t)(Y0 + y) * vp + Z0 + z);
-                r2[b] = *reinterpret_cast<const V2*>(job.u2 + (size_t)(Y0 + y) * pa + (size_t)(X0 + x) * vp + Z0 + z);
-            }
-            if (Z0 + z3 < v && X0 + x3 < v && Y0 + y3 < v)
-                r3[b] = *reinterpret_cast<const V2*>(job.u3 + (size_t)(Z0 + z3) * pa + (size_t)(X0 + x3) * vp + Y0 + y3);
-        }
-        // ---- small operands: (ov|ov) tiles, t1 rows, eps_v
-        const int occ[3] = {job.i, job.j, job.k};
-        for (int e = tid; e < 3 * 6 * 64; e += RED_THREADS) {
-            const int yy = e & 7, xx = (e >> 3) & 7, tp = (e >> 6) % 6, s = e / 384;
-            // ordered tile pairs (P,Q): (A,B),(A,C),(B,A),(B,C),(C,A),(C,B)
-            const int P = tp >> 1, Q = (tp & 1) ? (P == 2 ? 1 : 2) : (P == 0 ? 1 : 0);
-            const int o1 = (s == 0) ? occ[1] : occ[0];          // s=0: (j.|k.)  s=1: (i.|k.)  s=2: (i.|j.)
-            const int o2 = (s == 2) ? occ[1] : occ[2];
-            const int gx = tl[P] + xx, gy = tl[Q] + yy;
+// ---------------------------------------------------------------------------------------------- side pack
+// Per triplet of the batch: the three (ov|ov) slices  s=0: (j x|k y)  s=1: (i x|k y)  s=2: (i x|j y)  and the rows
+// t1[i], t1[j], t1[k], eps_v, cut into the tile-pair records the reduction copies; everything beyond v is zero.
+__global__ void __launch_bounds__(256)
+side_pack_kernel(const RedJob* __restrict__ jobs, int v, int o, int nt, const double* __restrict__ eps_v,
+                 const double* __restrict__ t1, const double* __restrict__ ovov, double* __restrict__ side) {
+    const RedJob job = jobs[blockIdx.y];
+    double* out = side + (size_t)job.slot * side_doubles(nt);
+    const int v8 = nt * 8;
+    const int nj = 3 * v8 * v8;
+    const int nrow = nt * nt * 64;          // (P, Q, which, row, x)
+    const int e = blockIdx.x * 256 + threadIdx.x;
+    if (e < nj) {
+        const int y = e % v8, x = (e / v8) % v8, s = e / (v8 * v8);
+        const int o1 = (s == 0) ? job.j : job.i;
+        const int o2 = (s == 2) ? job.j : job.k;
+        double val = 0.0;
+        if (x < v && y < v) val = ovov[(((size_t)o1 * v + x) * o + o2) * v + y];
+        const int P = x >> 3, Q = y >> 3, m = s * 64 + j_swz(x & 7, y & 7);
+        if (P <= Q) out[(size_t)(P * nt + Q) * RED_REC_DOUBLES + m] = val;             // J[P->Q] of rec[P][Q]
+        if (Q <= P) out[(size_t)(Q * nt + P) * RED_REC_DOUBLES + 192 + m] = val;       // J[Q'->P'] of rec[Q][P]
+    } else if (e < nj + nrow) {
+        const int f = e - nj;
+        const int xx = f & 7, row = (f >> 3) & 3, which = (f >> 5) & 1, pq = f >> 6;
+        const int P = pq / nt, Q = pq % nt;
+        if (P <= Q) {
+            const int x = (which ? Q : P) * 8 + xx;
             double val = 0.0;
-            if (gx < v && gy < v) val = ovov[(((size_t)o1 * v + gx) * o + o2) * v + gy];
-            Js[s][tp][xx][yy] = val;
+            if (x < v) val = row == 3 ? eps_v[x] : t1[(size_t)(row == 0 ? job.i : (row == 1 ? job.j : job.k)) * v + x];
+            out[(size_t)pq * RED_REC_DOUBLES + 384 + which * 32 + row * 8 + xx] = val;
         }
-        if (tid < 72) {
-            const int xx = tid & 7, tile = (tid >> 3) % 3, s = tid / 24;
-            const int gx = tl[tile] + xx;
-            T1s[s][tile][xx] = gx < v ? t1[(size_t)occ[s] * v + gx] : 0.0;
-        } else if (tid < 96) {
-            const int xx = tid & 7, tile = (tid - 72) >> 3;
-            const int gx = tl[tile] + xx;
-            Ev[tile][xx] = gx < v ? eps_v[gx] : 0.0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------- fused reduction
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// shared-memory loads with a compile-time displacement (one address register serves many loads)
+template <int IMM> __device__ __forceinline__ double lds64(uint32_t a) {
+    double x;
+    asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(x) : "r"(a), "n"(IMM));
+    return x;
+}
+template <int IMM> __device__ __forceinline__ int lds32i(uint32_t a) {
+    int x;
+    asm volatile("ld.shared.b32 %0, [%1+%2];" : "=r"(x) : "r"(a), "n"(IMM));
+    return x;
+}
+template <typename T, int IMM> __device__ __forceinline__ T ldsT(uint32_t a) {
+    if constexpr (sizeof(T) == 8) {
+        return lds64<IMM>(a);
+    } else {
+        float x;
+        asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(x) : "r"(a), "n"(IMM));
+        return x;
+    }
+}
+
+template <typename T> __device__ __forceinline__ double w_sum(T a, T b, T c);
+template <> __device__ __forceinline__ double w_sum<double>(double a, double b, double c) { return a + b + c; }
+// mixed path: W is a single-precision quantity: FP32 adds, promoted once
+template <> __device__ __forceinline__ double w_sum<float>(float a, float b, float c) {
+    return (double)__fadd_rn(__fadd_rn(a, b), c);
+}
+
+// W^{xyz} = U1[x,y,z] + U2[y,x,z] + U3[z,x,y] with (x,y,z) = arrangement PI of the thread's (a,b,c);
+// addr[pi] = stage base + byte offset of the thread's element inside a block read in arrangement pi.
+template <typename T, int PI>
+__device__ __forceinline__ double load_w(const uint32_t (&addr)[6]) {
+    using C = RedCfg<T>;
+    constexpr int P2 = arr_id(arr_y(PI), arr_x(PI), arr_z(PI));
+    constexpr int P3 = arr_id(arr_z(PI), arr_x(PI), arr_y(PI));
+    return w_sum<T>(ldsT<T, (PI * 3 + 0) * C::BLK_BYTES>(addr[PI]), ldsT<T, (P2 * 3 + 1) * C::BLK_BYTES>(addr[P2]),
+                    ldsT<T, (P3 * 3 + 2) * C::BLK_BYTES>(addr[P3]));
+}
+
+template <typename T>
+__global__ void __launch_bounds__(RED_THREADS, 1)
+reduce_kernel(const RedJob* __restrict__ jobs, int njobs, const uchar4* __restrict__ orbits, int norb, int v, int nt,
+              const double* __restrict__ eps_o, const double* __restrict__ side, double2* __restrict__ partials) {
+    using C = RedCfg<T>;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);     // keeps the shared address space
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + C::STAGES * C::STAGE_BYTES);
+    uint64_t* empty = full + C::STAGES;
+    const uint32_t smem_base = smem_u32(smem);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    if (tid == 0) {
+        for (int s = 0; s < C::STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], RED_CONSUMER_WARPS); }
+        fence_barrier_init();
+    }
+    __syncthreads();
+
+    if (warp == RED_CONSUMER_WARPS) {
+        // ------------------------------------------------------------------------------------ producer
+        const size_t sd = side_doubles(nt);
+        uint32_t it = 0;
+        for (int jb = blockIdx.y; jb < njobs; jb += gridDim.y) {
+            const RedJob job = jobs[jb];
+            const double eo = eps_o[job.i] + eps_o[job.j] + eps_o[job.k];
+            const double* sidej = side + (size_t)job.slot * sd;
+            for (int ob = blockIdx.x; ob < norb; ob += gridDim.x, ++it) {
+                const uchar4 orb = orbits[ob];
+                const int s = it % C::STAGES;
+                mbar_wait(&empty[s], ((it / C::STAGES) & 1) ^ 1);
+                const uint32_t st = smem_base + s * C::STAGE_BYTES;
+                if (lane == 0) {
+                    const double inv = orb.w == 1 ? 1.0 : (orb.w == 2 ? 0.5 : 1.0 / 6.0);
+                    asm volatile("st.shared.f64 [%0], %1;" ::"r"(st + C::H_OFF), "d"(eo) : "memory");
+                    asm volatile("st.shared.f64 [%0], %1;" ::"r"(st + C::H_OFF + 8), "d"(inv) : "memory");
+                    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(st + C::H_OFF + 16), "r"(orb.x * 8),
+                                 "r"(orb.y * 8), "r"(orb.z * 8), "r"(0)
+                                 : "memory");
+                    mbar_arrive_expect_tx(&full[s], C::TX_BYTES);   // release: the header is visible with the phase
+                }
+                __syncwarp();
+                const int tl0 = orb.x, tl1 = orb.y, tl2 = orb.z;
+                auto tile = [&](int which) { return which == 0 ? tl0 : (which == 1 ? tl1 : tl2); };
+                if (lane < 6) {                      // the three U blocks of arrangement `lane` of (A,B,C)
+                    const int X = tile(arr_x(lane)), Y = tile(arr_y(lane)), Z = tile(arr_z(lane));
+                    bulk_g2s(st + lane * 3 * C::BLK_BYTES,
+                             static_cast<const T*>(job.u) + ((size_t)(X * nt + Y) * nt + Z) * UCHUNK, 3 * C::BLK_BYTES,
+                             &full[s]);
+                } else if (lane < 9) {               // side records {A,B}, {A,C}, {B,C}
+                    const int r = lane - 6;
+                    const int P = tile(r == 2 ? 1 : 0), Q = tile(r == 0 ? 1 : 2);
+                    bulk_g2s(st + C::S_OFF + r * RED_REC_BYTES, sidej + (size_t)(P * nt + Q) * RED_REC_DOUBLES,
+                             RED_REC_BYTES, &full[s]);
+                }
+            }
         }
-        // ---- W = U1 + U2 (registers) -> smem, then += U3
-#pragma unroll
-        for (int b = 0; b < 6; ++b) {
-            double* dst = S + b * RBLK + x * RP2 + y * RP1 + z;
-            dst[0] = (double)r1[b].x + (double)r2[b].x;
-            dst[1] = (double)r1[b].y + (double)r2[b].y;
-        }
-        __syncthreads();
-#pragma unroll
-        for (int b = 0; b < 6; ++b) {
-            double* dst = S + b * RBLK + x3 * RP2 + y3 * RP1 + z3;
-            dst[0] += (double)r3[b].x;
-            dst[RP1] += (double)r3[b].y;
-        }
-        __syncthreads();
+        return;
     }
 
-    // ---- energy contraction over index triples (a in A, b in B, c in C)
-    const double eo = eps_o[job.i] + eps_o[job.j] + eps_o[job.k];
-    double e4 = 0.0, e5 = 0.0;
-    const int c = tid & 7, b = (tid >> 3) & 7;
+    // ---------------------------------------------------------------------------------------- consumers
+    // lane bits (c0,c1,b0,a0,b1), warp bits (c2,b2,a1); the two index triples of a thread differ in a2
+    const int c = (lane & 3) | ((warp & 1) << 2);
+    const int b = ((lane >> 2) & 1) | (((lane >> 4) & 1) << 1) | (((warp >> 1) & 1) << 2);
+    const int a_lo = ((lane >> 3) & 1) | (((warp >> 2) & 1) << 1);
+    // loop-invariant byte offsets of this thread's elements
+    uint32_t oU[2][6], qab[2], qba[2], qac[2], qca[2];
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
-        const int a = (tid >> 6) + 4 * h;
-        if (tl[0] + a < v && tl[1] + b < v && tl[2] + c < v) {
-            const double w0 = S[0 * RBLK + a * RP2 + b * RP1 + c];   // W^abc
-            const double w1 = S[1 * RBLK + a * RP2 + c * RP1 + b];   // W^acb
-            const double w2 = S[2 * RBLK + b * RP2 + a * RP1 + c];   // W^bac
-            const double w3 = S[3 * RBLK + b * RP2 + c * RP1 + a];   // W^bca
-            const double w4 = S[4 * RBLK + c * RP2 + a * RP1 + b];   // W^cab
-            const double w5 = S[5 * RBLK + c * RP2 + b * RP1 + a];   // W^cba
-            const double E = w0 + w3 + w4, O = w1 + w2 + w5;
-            const double q4 = 3.0 * (w0 * w0 + w1 * w1 + w2 * w2 + w3 * w3 + w4 * w4 + w5 * w5) + (E - O) * (E - O) -
-                              2.0 * E * O;
-            // Vd on the six permutations; Js[s][tp]: tp 0:(a,b) 1:(a,c) 2:(b,a) 3:(b,c) 4:(c,a) 5:(c,b)
-            const double ti_a = T1s[0][0][a], ti_b = T1s[0][1][b], ti_c = T1s[0][2][c];
-            const double tj_a = T1s[1][0][a], tj_b = T1s[1][1][b], tj_c = T1s[1][2][c];
-            const double tk_a = T1s[2][0][a], tk_b = T1s[2][1][b], tk_c = T1s[2][2][c];
-#define JJ(s, tp, x, y) Js[s][tp][x][y]
-            const double d0 = ti_a * JJ(0, 3, b, c) + tj_b * JJ(1, 1, a, c) + tk_c * JJ(2, 0, a, b);   // abc
-            const double d1 = ti_a * JJ(0, 5, c, b) + tj_c * JJ(1, 0, a, b) + tk_b * JJ(2, 1, a, c);   // acb
-            const double d2 = ti_b * JJ(0, 1, a, c) + tj_a * JJ(1, 3, b, c) + tk_c * JJ(2, 2, b, a);   // bac
-            const double d3 = ti_b * JJ(0, 4, c, a) + tj_c * JJ(1, 2, b, a) + tk_a * JJ(2, 3, b, c);   // bca
-            const double d4 = ti_c * JJ(0, 0, a, b) + tj_a * JJ(1, 5, c, b) + tk_b * JJ(2, 4, c, a);   // cab
-            const double d5 = ti_c * JJ(0, 2, b, a) + tj_b * JJ(1, 4, c, a) + tk_a * JJ(2, 5, c, b);   // cba
-#undef JJ
-            const double ze = E - 2.0 * O, zo = O - 2.0 * E;   // same-parity sum - 2 * other-parity sum
-            const double q5 = d0 * (3.0 * w0 + ze) + d3 * (3.0 * w3 + ze) + d4 * (3.0 * w4 + ze) +
-                              d1 * (3.0 * w1 + zo) + d2 * (3.0 * w2 + zo) + d5 * (3.0 * w5 + zo);
-            const double rD = 1.0 / (eo - Ev[0][a] - Ev[1][b] - Ev[2][c]);
-            e4 += q4 * rD;
-            e5 += q5 * rD;
+        const int idx[3] = {a_lo + 4 * h, b, c};
+#pragma unroll
+        for (int pi = 0; pi < 6; ++pi)
+            oU[h][pi] = (uint32_t)u_swz<C::ESZ>(idx[arr_x(pi)], idx[arr_y(pi)], idx[arr_z(pi)]) * C::ESZ;
+        qab[h] = j_swz(idx[0], b) * 8; qba[h] = j_swz(b, idx[0]) * 8;
+        qac[h] = j_swz(idx[0], c) * 8; qca[h] = j_swz(c, idx[0]) * 8;
+    }
+    const uint32_t qbc = j_swz(b, c) * 8, qcb = j_swz(c, b) * 8;
+
+    // ordered tile pair tp 0:(A,B) 1:(A,C) 2:(B,A) 3:(B,C) 4:(C,A) 5:(C,B) -> record {A,B}=0 {A,C}=1 {B,C}=2, half
+#define JREC(tp) ((tp) == 0 || (tp) == 2 ? 0 : ((tp) == 1 || (tp) == 4 ? 1 : 2))
+#define JHALF(tp) ((tp) == 2 || (tp) == 4 || (tp) == 5 ? 1 : 0)
+#define JJ(s, tp, areg) lds64<C::S_OFF + JREC(tp) * RED_REC_BYTES + JHALF(tp) * 1536 + (s) * 512>(areg)
+    // rows of tile A: record 0 first tile; B: record 0 second tile; C: record 1 second tile
+#define TT(tile, row, areg) \
+    lds64<C::S_OFF + ((tile) == 2 ? 1 : 0) * RED_REC_BYTES + 3072 + ((tile) == 0 ? 0 : 1) * 256 + (row) * 64>(areg)
+    uint32_t it = 0;
+    for (int jb = blockIdx.y; jb < njobs; jb += gridDim.y) {
+        double acc4 = 0.0, acc5 = 0.0;
+        for (int ob = blockIdx.x; ob < norb; ob += gridDim.x, ++it) {
+            const int s = it % C::STAGES;
+            mbar_wait(&full[s], (it / C::STAGES) & 1);
+            const uint32_t sb = smem_base + s * C::STAGE_BYTES;
+            const double eo = lds64<C::H_OFF>(sb), inv = lds64<C::H_OFF + 8>(sb);
+            const int A0 = lds32i<C::H_OFF + 16>(sb), B0 = lds32i<C::H_OFF + 20>(sb), C0 = lds32i<C::H_OFF + 24>(sb);
+            if (B0 + b < v && C0 + c < v) {
+                // quantities that do not depend on a
+                const uint32_t sb_b = sb + b * 8, sb_c = sb + c * 8;
+                const double ti_b = TT(1, 0, sb_b), tj_b = TT(1, 1, sb_b), tk_b = TT(1, 2, sb_b);
+                const double ti_c = TT(2, 0, sb_c), tj_c = TT(2, 1, sb_c), tk_c = TT(2, 2, sb_c);
+                const double ebc = eo - TT(1, 3, sb_b) - TT(2, 3, sb_c);
+                // J(s, tp, .): tp 0:(A,B) 1:(A,C) 2:(B,A) 3:(B,C) 4:(C,A) 5:(C,B)
+                const uint32_t abc_ = sb + qbc, acb_ = sb + qcb;
+                const double j0_bc = JJ(0, 3, abc_), j1_bc = JJ(1, 3, abc_), j2_bc = JJ(2, 3, abc_);
+                const double j0_cb = JJ(0, 5, acb_), j1_cb = JJ(1, 5, acb_), j2_cb = JJ(2, 5, acb_);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int a = a_lo + 4 * h;
+                    if (A0 + a < v) {
+                        uint32_t addr[6];
+#pragma unroll
+                        for (int pi = 0; pi < 6; ++pi) addr[pi] = sb + oU[h][pi];
+                        const double w0 = load_w<T, 0>(addr), w1 = load_w<T, 1>(addr), w2 = load_w<T, 2>(addr);
+                        const double w3 = load_w<T, 3>(addr), w4 = load_w<T, 4>(addr), w5 = load_w<T, 5>(addr);
+                        const double E = w0 + w3 + w4, O = w1 + w2 + w5;
+                        const double q4 = 3.0 * (w0 * w0 + w1 * w1 + w2 * w2 + w3 * w3 + w4 * w4 + w5 * w5) +
+                                          (E - O) * (E - O) - 2.0 * E * O;
+                        const uint32_t sb_a = sb + a * 8;
+                        const double ti_a = TT(0, 0, sb_a), tj_a = TT(0, 1, sb_a), tk_a = TT(0, 2, sb_a);
+                        const uint32_t aab = sb + qab[h], aba = sb + qba[h], aac = sb + qac[h], aca = sb + qca[h];
+                        const double d0 = ti_a * j0_bc + tj_b * JJ(1, 1, aac) + tk_c * JJ(2, 0, aab);           // abc
+                        const double d1 = ti_a * j0_cb + tj_c * JJ(1, 0, aab) + tk_b * JJ(2, 1, aac);           // acb
+                        const double d2 = ti_b * JJ(0, 1, aac) + tj_a * j1_bc + tk_c * JJ(2, 2, aba);           // bac
+                        const double d3 = ti_b * JJ(0, 4, aca) + tj_c * JJ(1, 2, aba) + tk_a * j2_bc;           // bca
+                        const double d4 = ti_c * JJ(0, 0, aab) + tj_a * j1_cb + tk_b * JJ(2, 4, aca);           // cab
+                        const double d5 = ti_c * JJ(0, 2, aba) + tj_b * JJ(1, 4, aca) + tk_a * j2_cb;           // cba
+                        const double ze = E - 2.0 * O, zo = O - 2.0 * E;   // same-parity sum - 2 * other-parity sum
+                        const double q5 = d0 * (3.0 * w0 + ze) + d3 * (3.0 * w3 + ze) + d4 * (3.0 * w4 + ze) +
+                                          d1 * (3.0 * w1 + zo) + d2 * (3.0 * w2 + zo) + d5 * (3.0 * w5 + zo);
+                        const double rD = inv / (ebc - TT(0, 3, sb_a));      // 1/sym folded into the reciprocal
+                        acc4 += q4 * rD;
+                        acc5 += q5 * rD;
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);     // this warp is done reading the stage
         }
-    }
-    // ---- deterministic block reduction: shuffle tree, then warp partials in index order
+        // ---- end of the triplet: shuffle tree inside the warp, one partial per (triplet, CTA column, warp)
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-        e4 += __shfl_xor_sync(0xffffffffu, e4, off);
-        e5 += __shfl_xor_sync(0xffffffffu, e5, off);
+        for (int off = 16; off > 0; off >>= 1) {
+            acc4 += __shfl_xor_sync(0xffffffffu, acc4, off);
+            acc5 += __shfl_xor_sync(0xffffffffu, acc5, off);
+        }
+        if (lane == 0)
+            partials[((size_t)jobs[jb].slot * gridDim.x + blockIdx.x) * RED_CONSUMER_WARPS + warp] =
+                make_double2(acc4, acc5);
     }
-    if ((tid & 31) == 0) { red[0][tid >> 5] = e4; red[1][tid >> 5] = e5; }
-    __syncthreads();
-    if (tid == 0) {
-        double s4 = 0.0, s5 = 0.0;
-#pragma unroll
-        for (int w = 0; w < RED_THREADS / 32; ++w) { s4 += red[0][w]; s5 += red[1][w]; }
-        const double inv = orb.w == 1 ? 1.0 : (orb.w == 2 ? 0.5 : 1.0 / 6.0);
-        partials[(size_t)job.slot * norb + blockIdx.x] = make_double2(s4 * inv, s5 * inv);
-    }
+#undef JJ
+#undef TT
+#undef JREC
+#undef JHALF
 }
 
 // One CTA per triplet of the batch: fixed-order sum of its orbit partials, weight w = 2 - d_ij - d_jk,
@@ -178,13 +319,13 @@ reduce_kernel(const RedJob<T>* __restrict__ jobs, const uchar4* __restrict__ orb
 struct FinJob { int slot; int index; double w; };
 
 __global__ void __launch_bounds__(128)
-finalize_kernel(const FinJob* __restrict__ jobs, const double2* __restrict__ partials, int norb,
+finalize_kernel(const FinJob* __restrict__ jobs, const double2* __restrict__ partials, int nper,
                 double* __restrict__ e_trip) {
     __shared__ double sh[2][128];
     const FinJob job = jobs[blockIdx.x];
-    const double2* p = partials + (size_t)job.slot * norb;
+    const double2* p = partials + (size_t)job.slot * nper;
     double s4 = 0.0, s5 = 0.0;
-    for (int n = threadIdx.x; n < norb; n += 128) { s4 += p[n].x; s5 += p[n].y; }
+    for (int n = threadIdx.x; n < nper; n += 128) { s4 += p[n].x; s5 += p[n].y; }
     sh[0][threadIdx.x] = s4; sh[1][threadIdx.x] = s5;
     __syncthreads();
     for (int st = 64; st > 0; st >>= 1) {
@@ -226,14 +367,12 @@ __global__ void __launch_bounds__(256) total_kernel(const double* __restrict__ e
 
 // W_out[a][b][c] = U1[a,b,c] + U2[b,a,c] + U3[c,a,b]  (test entry point triples_w_block; not on the hot path)
 template <typename T>
-__global__ void assemble_w_kernel(const T* __restrict__ u1, const T* __restrict__ u2, const T* __restrict__ u3, int v,
-                                  int vp, double* __restrict__ W) {
+__global__ void assemble_w_kernel(const T* __restrict__ u, int v, int nt, double* __restrict__ W) {
     const size_t n = (size_t)v * v * v;
-    const size_t pa = (size_t)v * vp;
     for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         const int c = (int)(e % v), b = (int)((e / v) % v), a = (int)(e / ((size_t)v * v));
-        W[e] = (double)u1[a * pa + (size_t)b * vp + c] + (double)u2[b * pa + (size_t)a * vp + c] +
-               (double)u3[c * pa + (size_t)a * vp + b];
+        W[e] = w_sum<T>(u[u_offset<sizeof(T)>(nt, a, b, c)], u[UBLK + u_offset<sizeof(T)>(nt, b, a, c)],
+                        u[2 * UBLK + u_offset<sizeof(T)>(nt, c, a, b)]);
     }
 }
 

@@ -5,6 +5,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -344,7 +345,7 @@ int run_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, c
         if (!(t.i == t.j && t.j == t.k)) work.push_back(t);
     const size_t nwork = work.size();
     std::vector<GemmJob> gj;
-    std::vector<RedJob<TS>> rj(nwork);
+    std::vector<RedJob> rj(nwork);
     std::vector<FinJob> fj(nwork);
     std::vector<int> gj_begin;   // first gemm job of each batch
     TS* ubase = reinterpret_cast<TS*>(ws + P.off_u);
@@ -353,25 +354,41 @@ int run_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, c
         const Triplet& t = work[n];
         const int slot = (int)(n % P.nb);
         if (slot == 0) gj_begin.push_back((int)gj.size());
-        TS* u1 = ubase + (size_t)(3 * slot + 0) * P.n_u;
-        TS* u2 = ubase + (size_t)(3 * slot + 1) * P.n_u;
-        TS* u3 = ubase + (size_t)(3 * slot + 2) * P.n_u;
-        gj.push_back({t.i, t.j, t.k, 0, u1});                       // G(i,j,k)[a][b][c]
-        if (t.i == t.j) u2 = u1; else gj.push_back({t.j, t.i, t.k, 0, u2});   // G(j,i,k)[b][a][c]
-        if (t.j == t.k) u3 = u2; else gj.push_back({t.k, t.i, t.j, 0, u3});   // G(k,i,j)[c][a][b]
+        TS* ub = ubase + (size_t)3 * slot * P.n_u;                 // interleaved blocks of U1,U2,U3 (ulayout.cuh)
+        TS *u1 = ub, *u2 = ub + UBLK, *u3 = ub + 2 * UBLK;
+        if (t.i == t.j) {            // G(j,i,k) = G(i,j,k): one job, two destinations
+            gj.push_back({t.i, t.j, t.k, 0, u1, u2});
+            gj.push_back({t.k, t.i, t.j, 0, u3, nullptr});
+        } else if (t.j == t.k) {     // G(k,i,j) = G(j,i,k)
+            gj.push_back({t.i, t.j, t.k, 0, u1, nullptr});
+            gj.push_back({t.j, t.i, t.k, 0, u2, u3});
+        } else {
+            gj.push_back({t.i, t.j, t.k, 0, u1, nullptr});               // G(i,j,k)[a][b][c]
+            gj.push_back({t.j, t.i, t.k, 0, u2, nullptr});               // G(j,i,k)[b][a][c]
+            gj.push_back({t.k, t.i, t.j, 0, u3, nullptr});               // G(k,i,j)[c][a][b]
+        }
         distinct_u += 1.0 + (t.i != t.j) + (t.j != t.k);
-        rj[n] = {t.i, t.j, t.k, slot, u1, u2, u3};
+        rj[n] = {t.i, t.j, t.k, slot, ub, nullptr};
         fj[n] = {slot, (int)t.index, triplet_weight(t.i, t.j, t.k)};
     }
     gj_begin.push_back((int)gj.size());
     GemmJob* d_gj = reinterpret_cast<GemmJob*>(ws + P.off_gjobs);
-    RedJob<TS>* d_rj = reinterpret_cast<RedJob<TS>*>(ws + P.off_rjobs);
+    RedJob* d_rj = reinterpret_cast<RedJob*>(ws + P.off_rjobs);
+    double* d_side = reinterpret_cast<double*>(ws + P.off_side);
+    static_assert(kRedWarps == RED_CONSUMER_WARPS, "plan.h and reduce.cuh disagree");
+    {
+        static bool attr_set = false;
+        if (!attr_set) {
+            CU_TRY(cudaFuncSetAttribute(reduce_kernel<TS>, cudaFuncAttributeMaxDynamicSharedMemorySize, RedCfg<TS>::SMEM_BYTES));
+            attr_set = true;
+        }
+    }
     FinJob* d_fj = reinterpret_cast<FinJob*>(ws + P.off_fjobs);
     uchar4* d_orb = reinterpret_cast<uchar4*>(ws + P.off_orb);
     double2* d_part = reinterpret_cast<double2*>(ws + P.off_part);
     if (!gj.empty()) CU_TRY(cudaMemcpyAsync(d_gj, gj.data(), gj.size() * sizeof(GemmJob), cudaMemcpyHostToDevice, st));
     if (nwork) {
-        CU_TRY(cudaMemcpyAsync(d_rj, rj.data(), nwork * sizeof(RedJob<TS>), cudaMemcpyHostToDevice, st));
+        CU_TRY(cudaMemcpyAsync(d_rj, rj.data(), nwork * sizeof(RedJob), cudaMemcpyHostToDevice, st));
         CU_TRY(cudaMemcpyAsync(d_fj, fj.data(), nwork * sizeof(FinJob), cudaMemcpyHostToDevice, st));
     }
     CU_TRY(cudaMemcpyAsync(d_orb, orbits.data(), orbits.size() * sizeof(Orbit), cudaMemcpyHostToDevice, st));
@@ -391,12 +408,20 @@ int run_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, c
         }
         if (int rc = launch_gemm(P, maps, d_gj + g0, g1 - g0, st)) return rc;
         if (prof) CU_TRY(cudaEventRecord(e[1], st));
-        reduce_kernel<TS><<<dim3(P.norb, cnt), RED_THREADS, 0, st>>>(d_rj + n0, d_orb, P.norb, v, P.vp, o, in.eps_o,
-                                                                      in.eps_v, in.t1, in.ovov, d_part);
-        CU_TRY(cudaGetLastError());
-        ++g_launches;
+        {
+            const int v8 = P.nt * 8;
+            dim3 grid((3 * v8 * v8 + P.nt * P.nt * 64 + 255) / 256, cnt);
+            side_pack_kernel<<<grid, 256, 0, st>>>(d_rj + n0, v, o, P.nt, in.eps_v, in.t1, in.ovov, d_side);
+            CU_TRY(cudaGetLastError());
+            ++g_launches;
+            const int gy = std::max(1, std::min(cnt, kNumSM / P.red_gx));
+            reduce_kernel<TS><<<dim3(P.red_gx, gy), RED_THREADS, RedCfg<TS>::SMEM_BYTES, st>>>(
+                d_rj + n0, cnt, d_orb, P.norb, v, P.nt, in.eps_o, d_side, d_part);
+            CU_TRY(cudaGetLastError());
+            ++g_launches;
+        }
         if (prof) CU_TRY(cudaEventRecord(e[2], st));
-        finalize_kernel<<<cnt, 128, 0, st>>>(d_fj + n0, d_part, P.norb, e_trip);
+        finalize_kernel<<<cnt, 128, 0, st>>>(d_fj + n0, d_part, P.red_gx * kRedWarps, e_trip);
         CU_TRY(cudaGetLastError());
         ++g_launches;
         if (prof) {
@@ -596,17 +621,15 @@ int triples_w_block(int nocc, int nvirt, const double* t2, const double* vvvo, c
     Maps maps;
     if (int rc = build_maps(P, op, &maps)) return rc;
     uint8_t* ubase = ws + P.off_u;
-    const size_t ub = P.n_u * P.esz;   // bytes of one U buffer
-    GemmJob gj[3] = {{i, j, k, 0, ubase}, {j, i, k, 0, ubase + ub}, {k, i, j, 0, ubase + 2 * ub}};
+    const size_t ub = (size_t)UBLK * P.esz;   // U1, U2, U3 blocks of a tile are adjacent
+    GemmJob gj[3] = {{i, j, k, 0, ubase, nullptr}, {j, i, k, 0, ubase + ub, nullptr}, {k, i, j, 0, ubase + 2 * ub, nullptr}};
     GemmJob* d_gj = reinterpret_cast<GemmJob*>(ws + P.off_gjobs);
     CU_TRY(cudaMemcpyAsync(d_gj, gj, sizeof gj, cudaMemcpyHostToDevice, st));
     if (int rc = launch_gemm(P, maps, d_gj, 3, st)) return rc;
     if (precision == TRIPLES_FP64)
-        assemble_w_kernel<double><<<kNumSM * 4, 256, 0, st>>>((const double*)ubase, (const double*)(ubase + ub),
-                                                               (const double*)(ubase + 2 * ub), nvirt, P.vp, W_out);
+        assemble_w_kernel<double><<<kNumSM * 4, 256, 0, st>>>((const double*)ubase, nvirt, P.nt, W_out);
     else
-        assemble_w_kernel<float><<<kNumSM * 4, 256, 0, st>>>((const float*)ubase, (const float*)(ubase + ub),
-                                                              (const float*)(ubase + 2 * ub), nvirt, P.vp, W_out);
+        assemble_w_kernel<float><<<kNumSM * 4, 256, 0, st>>>((const float*)ubase, nvirt, P.nt, W_out);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     CU_TRY(cudaStreamSynchronize(st));
