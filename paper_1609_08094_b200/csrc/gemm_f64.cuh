@@ -24,10 +24,14 @@
 namespace tb {
 
 struct GemmJob {
-    int p, q, r, pad;
+    int p, q, r;
+    int gstart;  // jobs of a batch are sorted by (q,r); [gstart, gstart + gsize) = the jobs sharing this job's (q,r),
     void* out;   // G(p,q,r)[a][b][c] in the blocked layout of ulayout.cuh: slot base + u * UBLK
     void* out2;  // second destination (or null): a triplet with i=j or j=k uses the same G twice
+    int gsize;   // i.e. the same X_r / XT_q operand slices: walked tile by tile together
+    int pad[3];
 };
+static_assert(sizeof(GemmJob) == 48, "plan.h sizes the job table with 48 bytes per job");
 
 struct alignas(64) GemmMaps {
     CUtensorMap t2a;   // t2 as A: (d, a, pq)          box (16, BM, 1)

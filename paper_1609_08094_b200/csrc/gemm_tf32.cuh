@@ -15,10 +15,17 @@
 // T2A[p][q][a][d] = t2, OtA[r][p][a][l] = -(pa|lr), T2K[q][b][c][l] = t2[q,l,b,c], T2KT[r][b][c][l] = t2[l,r,b,c];
 // the c index has vp rows per b (row v is zero when v is odd) so that U keeps the pitch the reduction expects.
 //
-// One CTA (persistent, one per SM) walks work items (job, m-tile of 128 (b,c) rows, n-tile of BN a-columns):
-//   warp 0    : TMA producer   (K chunks of 32 floats = one 128-byte swizzled row per operand row; hi and lo tiles)
-//   warp 1    : MMA issuer     (one lane; per K chunk: 4 k-steps of lo*hi and hi*lo, then 4 k-steps of hi*hi)
-//   warp 2    : TMEM allocator (512 columns = two 128 x 256 FP32 buffers)
+// The kernel is persistent and runs as CTA PAIRS (thread-block clusters of 2 = the two SMs of a TPC, cta_group::2):
+// a pair walks work items (job, two consecutive m-tiles of 128 (b,c) rows, n-tile of BN a-columns) as ONE
+// 256 x BN MMA tile.  Each CTA stages only its own 128 M-side rows and HALF of the N-side rows (the tensor cores
+// read the other half from the peer's shared memory), which cuts the bytes every SM has to pull in per MMA by a
+// third: with hi+lo operands (8 bytes per element) the single-CTA tile was bound by the ~40 B/clk an SM can ingest
+// from L2, not by the tensor pipe (round-1 ncu: tensor pipe 47 % active, 8.4 TB/s L2->SM).
+//   warp 0    : TMA producer   (K chunks of 32 floats = one 128-byte swizzled row per operand row; hi and lo tiles;
+//                               both CTAs load, the transaction bytes all count on the leader's barrier)
+//   warp 1    : MMA issuer     (one lane of the LEADER CTA; per K chunk: 4 k-steps of lo*hi and hi*lo, then 4
+//                               k-steps of hi*hi; tcgen05.commit multicasts to both CTAs' barriers)
+//   warp 2    : TMEM allocator (512 columns = two 128 x 256 FP32 buffers in each CTA)
 //   warps 4-11: accumulators   (tcgen05.ld of every finished chain, FP32 round-to-nearest adds in registers,
 //                               coalesced FP32 stores of U[a][(b,c)] at the end of the tile)
 //
@@ -52,22 +59,35 @@ constexpr int TF_TMEM_COLS = 512;
 constexpr int TF_MAX_STAGES = 4;
 constexpr int TF_SMEM_LIMIT = 227 * 1024;
 
-__host__ __device__ constexpr int tf32_stage_bytes(int bn) { return 2 * TF_BM * 128 + 2 * bn * 128; }
-// stages that fit (>= 2 for every bn <= 256), capped; the dynamic smem request is always > half an SM's shared
+// npad = N-side rows a CTA stages: bn / 2 in pair mode (cs = 2), bn for a single CTA (cs = 1)
+__host__ __device__ constexpr int tf32_stage_bytes(int npad) { return 2 * TF_BM * 128 + 2 * npad * 128; }
+// stages that fit (>= 2 for every npad <= 256), capped; the dynamic smem request is always > half an SM's shared
 // memory so that exactly one CTA is resident per SM (it owns all 512 TMEM columns).
-__host__ __device__ constexpr int tf32_stages(int bn) {
-    int s = (TF_SMEM_LIMIT - 2048) / tf32_stage_bytes(bn);
+__host__ __device__ constexpr int tf32_stages(int npad) {
+    int s = (TF_SMEM_LIMIT - 2048) / tf32_stage_bytes(npad);
     return s > TF_MAX_STAGES ? TF_MAX_STAGES : s;
 }
-__host__ __device__ constexpr int tf32_smem_bytes(int bn) { return tf32_stages(bn) * tf32_stage_bytes(bn) + 2048; }
+__host__ __device__ constexpr int tf32_smem_bytes(int npad) { return tf32_stages(npad) * tf32_stage_bytes(npad) + 2048; }
+
+// Work item w -> (job, tile).  The jobs of a launch are sorted by (q,r) (triples_b200.cu); the gsize jobs of a group
+// share their M-side operand slices XK_r / XKT_q / T2K_q / T2KT_r, so consecutive items are the SAME tile of the
+// group's jobs: the CTAs running side by side then pull identical M-side rows, and the (vv|vo) slices come from HBM
+// once per group instead of once per job (they are far larger than L2: 2 x v^3 x 8 bytes per job).
+__device__ __forceinline__ void tf32_item(const GemmJob* __restrict__ jobs, long long w, int per_job, int& jb, int& rem) {
+    const int any = (int)(w / per_job);                       // some job of the group item w falls in
+    const int gs = jobs[any].gstart, gn = jobs[any].gsize;
+    const long long local = w - (long long)gs * per_job;
+    jb = gs + (int)(local % gn);
+    rem = (int)(local / gn);
+}
 
 __global__ void __launch_bounds__(TF_THREADS, 1)
 gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restrict__ jobs, int njobs, int v, int vp,
-                 int o, int mtiles, int ntiles, int bn) {
+                 int o, int mtiles, int ntiles, int bn, int cs, int npad, int dbg) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    const int stages = tf32_stages(bn);
-    const int stage_bytes = tf32_stage_bytes(bn);
+    const int stages = tf32_stages(npad);
+    const int stage_bytes = tf32_stage_bytes(npad);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem + stages * stage_bytes);
     uint64_t* empty = full + TF_MAX_STAGES;
     uint64_t* tfull = empty + TF_MAX_STAGES;     // accumulator buffer ready for the epilogue
@@ -76,20 +96,28 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nrows = v * vp;                                   // flattened (b,c') rows
-    const int per_job = mtiles * ntiles;
+    // a pair (cs = 2) walks two consecutive m-tiles of one (job, n-tile) as one 256-row MMA tile
+    const int rank = cs > 1 ? (int)cluster_ctarank() : 0;
+    const int cid = blockIdx.x / cs, ncl = gridDim.x / cs;
+    const int per_job = ((mtiles + cs - 1) / cs) * ntiles;
     const long long nitems = (long long)njobs * per_job;
     const int kst_v = (v + 7) >> 3, kst_o = (o + 7) >> 3;       // 8-wide k-steps per segment
     const int nch_v = (v + TF_BK - 1) / TF_BK, nch_o = (o + TF_BK - 1) / TF_BK;
     const int nch = 2 * (nch_v + nch_o);
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
-        for (int b = 0; b < 2; ++b) { mbar_init(&tfull[b], 1); mbar_init(&tempty[b], 8); }
+        // full / tempty are waited on by the leader's MMA thread only: both CTAs' producers (accumulator warps) arrive
+        for (int s = 0; s < stages; ++s) { mbar_init(&full[s], cs); mbar_init(&empty[s], 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(&tfull[b], 1); mbar_init(&tempty[b], 8 * cs); }
         fence_barrier_init();
     }
-    if (warp == 2) { tmem_alloc(tmem_slot, TF_TMEM_COLS); tmem_relinquish(); }
+    if (warp == 2) {
+        if (cs == 1) { tmem_alloc(tmem_slot, TF_TMEM_COLS); tmem_relinquish(); }
+        else { tmem_alloc_pair(tmem_slot, TF_TMEM_COLS); tmem_relinquish_pair(); }
+    }
     tc_fence_before_sync();
     __syncthreads();
+    if (cs > 1) cluster_sync_all();     // every CTA's barriers are initialised before a peer's TMA / commit reaches them
     tc_fence_after_sync();
     const uint32_t tmem_base = *tmem_slot;
 
@@ -102,37 +130,54 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                 tma_prefetch_desc(&maps.t2kt[h]); tma_prefetch_desc(&maps.t2a[h]); tma_prefetch_desc(&maps.ota[h]);
             }
             uint32_t it = 0;
-            for (long long w = blockIdx.x; w < nitems; w += gridDim.x) {
-                const int jb = (int)(w / per_job), rem = (int)(w % per_job);
-                const int m0 = (rem / ntiles) * TF_BM, a0 = (rem % ntiles) * bn;
+            for (long long w = cid; w < nitems; w += ncl) {
+                int jb, rem;
+                tf32_item(jobs, w, per_job, jb, rem);
+                int m0 = ((rem / ntiles) * cs + rank) * TF_BM;
+                const int a0 = (rem % ntiles) * bn;
                 const GemmJob job = jobs[jb];
                 const int p = job.p, q = job.q, r = job.r;
                 for (int c = 0; c < nch; ++c, ++it) {
                     const int s = it % stages;
                     mbar_wait(&empty[s], ((it / stages) & 1) ^ 1);
                     uint8_t* sM = smem + s * stage_bytes;           // [hi 128 rows][lo 128 rows]
-                    uint8_t* sN = sM + 2 * TF_BM * 128;             // [hi bn rows][lo bn rows]
-                    mbar_arrive_expect_tx(&full[s], stage_bytes);
+                    uint8_t* sN = sM + 2 * TF_BM * 128;             // [hi npad rows][lo npad rows]
+                    if (rank == 0 && !(dbg & 4)) mbar_arrive_expect_tx(&full[s], cs * stage_bytes);
                     const CUtensorMap *mm, *nm;
                     int kk, mz, nz;
                     if (c < nch_v)                     { kk = c * TF_BK;                       mm = maps.xk;   mz = r; nm = maps.t2a; nz = p * o + q; }
                     else if (c < 2 * nch_v)            { kk = (c - nch_v) * TF_BK;             mm = maps.xkt;  mz = q; nm = maps.t2a; nz = p * o + r; }
                     else if (c < 2 * nch_v + nch_o)    { kk = (c - 2 * nch_v) * TF_BK;         mm = maps.t2k;  mz = q; nm = maps.ota; nz = r * o + p; }
                     else                               { kk = (c - 2 * nch_v - nch_o) * TF_BK; mm = maps.t2kt; mz = r; nm = maps.ota; nz = q * o + p; }
-                    tma_load_3d(sM, &mm[0], &full[s], kk, m0, mz);
-                    tma_load_3d(sM + TF_BM * 128, &mm[1], &full[s], kk, m0, mz);
-                    tma_load_3d(sN, &nm[0], &full[s], kk, a0, nz);
-                    tma_load_3d(sN + bn * 128, &nm[1], &full[s], kk, a0, nz);
+                    if (dbg & 8) { kk = 0; mz = 0; nz = 0; }
+                    if (dbg & 4) {
+                        if (rank == 0) mbar_arrive(&full[s]);
+                        else mbar_arrive_cluster(mapa_u32(smem_u32(&full[s]), 0));
+                    } else if (cs == 1) {
+                        tma_load_3d(sM, &mm[0], &full[s], kk, m0, mz);
+                        tma_load_3d(sM + TF_BM * 128, &mm[1], &full[s], kk, m0, mz);
+                        tma_load_3d(sN, &nm[0], &full[s], kk, a0, nz);
+                        tma_load_3d(sN + npad * 128, &nm[1], &full[s], kk, a0, nz);
+                    } else {   // own M rows, own half of the N rows; every byte is counted on the leader's barrier
+                        const uint32_t lbar = mapa_u32(smem_u32(&full[s]), 0);
+                        if (rank != 0) mbar_arrive_cluster(lbar);
+                        const int an = a0 + rank * npad;
+                        if (dbg & 8) m0 = 0;
+                        tma_load_3d_pair(sM, &mm[0], lbar, kk, m0, mz);
+                        tma_load_3d_pair(sM + TF_BM * 128, &mm[1], lbar, kk, m0, mz);
+                        tma_load_3d_pair(sN, &nm[0], lbar, kk, an, nz);
+                        tma_load_3d_pair(sN + npad * 128, &nm[1], lbar, kk, an, nz);
+                    }
                 }
             }
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------------------------------ MMA issuer
-        if (lane == 0) {
-            const uint32_t idesc = umma_idesc_tf32_m128((uint32_t)bn);
+        if (lane == 0 && rank == 0) {
+            const uint32_t idesc = cs == 1 ? umma_idesc_tf32_m128((uint32_t)bn) : umma_idesc_tf32_m256((uint32_t)bn);
             const uint32_t smem_base = smem_u32(smem);
             uint32_t it = 0, chain = 0;
-            for (long long w = blockIdx.x; w < nitems; w += gridDim.x) {
+            for (long long w = cid; w < nitems; w += ncl) {
                 for (int c = 0; c < nch; ++c, ++it) {
                     const int s = it % stages;
                     int left;   // k-steps of this chunk that carry data
@@ -153,20 +198,35 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                     const uint32_t sM = smem_base + s * stage_bytes;
                     const uint32_t sN = sM + 2 * TF_BM * 128;
                     const uint64_t mh = umma_desc_sw128(sM), ml = umma_desc_sw128(sM + TF_BM * 128);
-                    const uint64_t nh = umma_desc_sw128(sN), nl = umma_desc_sw128(sN + bn * 128);
+                    const uint64_t nh = umma_desc_sw128(sN), nl = umma_desc_sw128(sN + npad * 128);
                     uint32_t acc = first ? 0u : 1u;
-                    for (int k = 0; k < nk; ++k) {                   // small terms first
-                        const uint64_t adv = (uint64_t)(k * 2);      // 32 bytes per k-step, in 16-byte units
-                        umma_tf32(tacc, ml + adv, nh + adv, idesc, acc);      // lo*hi
-                        acc = 1;
-                        umma_tf32(tacc, mh + adv, nl + adv, idesc, 1);        // hi*lo
+                    if (cs == 1) {
+                        for (int k = 0; k < nk; ++k) {                   // small terms first
+                            const uint64_t adv = (uint64_t)(k * 2);      // 32 bytes per k-step, in 16-byte units
+                            umma_tf32(tacc, ml + adv, nh + adv, idesc, acc);      // lo*hi
+                            acc = 1;
+                            umma_tf32(tacc, mh + adv, nl + adv, idesc, 1);        // hi*lo
+                        }
+                        for (int k = 0; k < nk; ++k) {
+                            const uint64_t adv = (uint64_t)(k * 2);
+                            umma_tf32(tacc, mh + adv, nh + adv, idesc, 1);        // hi*hi
+                        }
+                        umma_commit(&empty[s]);       // smem slot free once these MMAs have read it
+                        if (last) { umma_commit(&tfull[buf]); ++chain; }   // chain complete
+                    } else {
+                        for (int k = 0; k < nk; ++k) {
+                            const uint64_t adv = (uint64_t)(k * 2);
+                            umma_tf32_pair(tacc, ml + adv, nh + adv, idesc, acc);
+                            acc = 1;
+                            umma_tf32_pair(tacc, mh + adv, nl + adv, idesc, 1);
+                        }
+                        for (int k = 0; k < nk; ++k) {
+                            const uint64_t adv = (uint64_t)(k * 2);
+                            umma_tf32_pair(tacc, mh + adv, nh + adv, idesc, 1);
+                        }
+                        umma_commit_pair(&empty[s]);                       // both CTAs' slots
+                        if (last) { umma_commit_pair(&tfull[buf]); ++chain; }   // both CTAs' accumulator warps
                     }
-                    for (int k = 0; k < nk; ++k) {
-                        const uint64_t adv = (uint64_t)(k * 2);
-                        umma_tf32(tacc, mh + adv, nh + adv, idesc, 1);        // hi*hi
-                    }
-                    umma_commit(&empty[s]);       // smem slot free once these MMAs have read it
-                    if (last) { umma_commit(&tfull[buf]); ++chain; }   // chain complete
                 }
             }
         }
@@ -178,9 +238,10 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
         const int nchain = (nch + TF_CHAIN - 1) / TF_CHAIN;
         const bool active = half * 128 < bn;
         uint32_t chain = 0;
-        for (long long w = blockIdx.x; w < nitems; w += gridDim.x) {
-            const int jb = (int)(w / per_job), rem = (int)(w % per_job);
-            const int m0 = (rem / ntiles) * TF_BM, a0 = (rem % ntiles) * bn;
+        for (long long w = cid; w < nitems; w += ncl) {
+            int jb, rem;
+            tf32_item(jobs, w, per_job, jb, rem);
+            const int m0 = ((rem / ntiles) * cs + rank) * TF_BM, a0 = (rem % ntiles) * bn;
             float acc[128];
 #pragma unroll
             for (int j = 0; j < 128; ++j) acc[j] = 0.0f;
@@ -188,7 +249,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                 const uint32_t buf = chain & 1;
                 mbar_wait(&tfull[buf], (chain >> 1) & 1);
                 tc_fence_after_sync();
-                if (active) {
+                if (active && !(dbg & 2)) {
                     const uint32_t taddr = tmem_base + buf * 256 + half * 128 + ((uint32_t)(wq * 32) << 16);
 #pragma unroll
                     for (int c0 = 0; c0 < 128; c0 += 16) {
@@ -201,12 +262,15 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                 }
                 tc_fence_before_sync();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&tempty[buf]);
+                if (lane == 0) {     // the leader's MMA thread owns the buffer hand-back of both CTAs
+                    if (cs == 1) mbar_arrive(&tempty[buf]);
+                    else mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[buf]), 0));
+                }
             }
             // blocked + swizzled store (ulayout.cuh): this thread owns (b,c) = row, the columns are a
             const int row = m0 + wq * 32 + lane;
             const int bb = row / vp, cc = row - bb * vp;
-            if (active && row < nrows && cc < v) {
+            if (active && row < nrows && cc < v && !(dbg & 1)) {
                 float* __restrict__ out = static_cast<float*>(jobs[jb].out);
                 float* __restrict__ out2 = static_cast<float*>(jobs[jb].out2);
                 const int nt = u_tiles(v);
@@ -226,7 +290,11 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
     }
     tc_fence_before_sync();
     __syncthreads();
-    if (warp == 2) { tc_fence_after_sync(); tmem_dealloc(tmem_base, TF_TMEM_COLS); }
+    if (cs > 1) cluster_sync_all();     // no CTA leaves while a peer may still write its shared memory or barriers
+    if (warp == 2) {
+        tc_fence_after_sync();
+        if (cs == 1) tmem_dealloc(tmem_base, TF_TMEM_COLS); else tmem_dealloc_pair(tmem_base, TF_TMEM_COLS);
+    }
 }
 
 }  // namespace tb

@@ -3,6 +3,7 @@
 #pragma once
 #include <cstddef>
 #include <cstdint>
+#include <cstdlib>
 #include <vector>
 
 namespace tb {
@@ -54,12 +55,21 @@ inline void enumerate_orbits(int v, std::vector<Orbit>& out) {
 
 enum GemmCfgId { CFG_M120_N128 = 0, CFG_M80_N192 = 1, CFG_M40_N256 = 2 };
 
+// CTAs per MMA tile of the mixed contraction: 2 = CTA pair (default), 1 = single CTA; TRIPLES_TF_CLUSTER=1 selects
+// the single-CTA variant for A/B measurements.
+inline int tf_cluster_size() {
+    if (const char* e = std::getenv("TRIPLES_TF_CLUSTER")) return std::atoi(e) == 1 ? 1 : 2;
+    return 2;
+}
+
 struct Plan {
     int o = 0, v = 0, vp = 0, op = 0, prec = 0;
     int vk = 0, ok = 0;         // mixed path: K pitches of the K-major FP32 operands (v, o rounded up to 4)
     int cfg = 0, BM = 0, BN = 0, mtiles = 0, ntiles = 0;      // FP64 contraction tiles
     int tf_bn = 0, tf_ntiles = 0, tf_mtiles = 0;              // mixed contraction tiles: 128 (b,c) rows x tf_bn a-columns
-    int nb = 0;                 // triplets per batch
+    int tf_cs = 1, tf_npad = 0;                               // CTAs per MMA tile (2 = cta_group::2 pair); N-side rows a CTA stages
+    int nb = 0;                 // triplets per batch (at most win^3)
+    int win = 1;                // batch = block of occupied-index windows of this width (see make_plan)
     long long T = 0;            // restricted triplets
     int norb = 0, nt = 0;       // tile orbits, 8-wide tiles per virtual axis
     int red_gx = 0;             // CTA columns of the fused reduction (orbit stride), fixed by v
@@ -118,20 +128,29 @@ inline bool make_plan(int o, int v, int prec, Plan& P) {
         P.tf_ntiles = (v + 255) / 256;
         P.tf_bn = (((v + P.tf_ntiles - 1) / P.tf_ntiles) + 15) & ~15;
         P.tf_mtiles = (int)((N + 127) / 128);
+        // CTA pairs (cta_group::2): a pair owns two consecutive m-tiles, each CTA stages half of the N-side rows
+        // (tf_bn is a multiple of 16, so a half is whole 8-row swizzle atoms)
+        P.tf_cs = tf_cluster_size();
+        P.tf_npad = P.tf_bn / P.tf_cs;
         P.n_x = (size_t)o * v * P.vp * P.vk;
         P.n_t2 = (size_t)o * o * v * P.vk;
         P.n_ot = (size_t)o * o * v * P.ok;
         P.n_t2k = (size_t)o * v * P.vp * P.ok;
-        ctas_per_triplet = 3LL * P.tf_mtiles * P.tf_ntiles;
+        ctas_per_triplet = 3LL * ((P.tf_mtiles + P.tf_cs - 1) / P.tf_cs) * P.tf_cs * P.tf_ntiles;
         waves = 60;
     }
-    // batch: enough CTAs for >= `waves` waves of 148 SMs, U buffers capped at 12 GiB, at least one triplet
-    long long nb = (waves * kNumSM + ctas_per_triplet - 1) / ctas_per_triplet;
-    const long long cap = (long long)((12ULL << 30) / (3 * P.n_u * P.esz));
-    if (nb > cap) nb = cap;
+    // Batch = all restricted triplets of one block I x J x K of occupied-index windows of width `win` (S1).  Inside
+    // a block every contraction job (p; q,r) has win - 1 siblings with the same (q,r), i.e. the same X_r / XT_q
+    // slices, which the contraction kernels walk tile by tile together: the big (vv|vo) operand then comes from HBM
+    // once per group instead of once per job.  win: as wide as the U buffers allow (22 GiB cap,
+    // sized for the 180 GB part next to 2 x 35 GB of repacked integrals at the largest config), at most 4.
+    (void)ctas_per_triplet; (void)waves;
+    const long long cap = (long long)((22ULL << 30) / (3 * P.n_u * P.esz));
+    int win = 1;
+    while (win < 4 && win < o && (long long)(win + 1) * (win + 1) * (win + 1) <= cap) ++win;
+    P.win = win;
+    long long nb = (long long)win * win * win;
     if (nb > P.T) nb = P.T;
-    if (nb > 20000) nb = 20000;   // gridDim.y limit of the contraction launch (3 jobs per triplet)
-    if (nb < 1) nb = 1;
     P.nb = (int)nb;
 
     size_t off = 0;
@@ -156,7 +175,7 @@ inline bool make_plan(int o, int v, int prec, Plan& P) {
     P.off_side = take((size_t)P.nb * P.n_side * 8);
     P.off_etrip = take((size_t)P.T * 3 * 8);
     P.off_result = take(256);
-    P.off_gjobs = take((size_t)P.T * 3 * 32);
+    P.off_gjobs = take((size_t)P.T * 3 * 48);
     P.off_rjobs = take((size_t)P.T * 48);
     P.off_fjobs = take((size_t)P.T * 16);
     P.off_orb = take((size_t)P.norb * 4);

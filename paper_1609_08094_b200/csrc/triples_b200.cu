@@ -168,8 +168,8 @@ int build_maps_tf32(const Plan& P, const Operands& op, Tf32Maps* maps) {
         if ((rc = make_map3(&maps->xkt[h], dt, 4, xkt[h], v, NR, o, vk, NR * vk, TF_BK, TF_BM, 1))) return rc;
         if ((rc = make_map3(&maps->t2k[h], dt, 4, t2k[h], o, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
         if ((rc = make_map3(&maps->t2kt[h], dt, 4, t2kt[h], o, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
-        if ((rc = make_map3(&maps->t2a[h], dt, 4, t2a[h], v, v, o * o, vk, v * vk, TF_BK, P.tf_bn, 1))) return rc;
-        if ((rc = make_map3(&maps->ota[h], dt, 4, ota[h], o, v, o * o, ok, v * ok, TF_BK, P.tf_bn, 1))) return rc;
+        if ((rc = make_map3(&maps->t2a[h], dt, 4, t2a[h], v, v, o * o, vk, v * vk, TF_BK, P.tf_npad, 1))) return rc;
+        if ((rc = make_map3(&maps->ota[h], dt, 4, ota[h], o, v, o * o, ok, v * ok, TF_BK, P.tf_npad, 1))) return rc;
     }
     return TRIPLES_OK;
 }
@@ -184,12 +184,37 @@ int launch_gemm_tf32(const Tf32Maps& maps, const GemmJob* jobs, int njobs, const
         CU_TRY(cudaFuncSetAttribute(gemm_tf32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TF_SMEM_LIMIT));
         attr_set = true;
     }
-    const long long items = (long long)njobs * P.tf_mtiles * P.tf_ntiles;
+    const int cs = P.tf_cs;
+    const long long items = (long long)njobs * ((P.tf_mtiles + cs - 1) / cs) * P.tf_ntiles;   // per cluster
     if (items == 0) return TRIPLES_OK;
-    const int grid = (int)std::min<long long>(items, kNumSM);
-    gemm_tf32_kernel<<<grid, TF_THREADS, tf32_smem_bytes(P.tf_bn), st>>>(maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles,
-                                                                        P.tf_ntiles, P.tf_bn);
-    CU_TRY(cudaGetLastError());
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cs; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.blockDim = dim3(TF_THREADS);
+    cfg.dynamicSmemBytes = tf32_smem_bytes(P.tf_npad);
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = cs > 1 ? 1 : 0;
+    static const int dbg = std::getenv("TRIPLES_TF_DEBUG") ? std::atoi(std::getenv("TRIPLES_TF_DEBUG")) : 0;
+    static int max_clusters[5] = {0, 0, 0, 0, 0};   // co-resident clusters of this size (one CTA per SM)
+    if (cs == 1) max_clusters[1] = kNumSM;
+    if (!max_clusters[cs]) {
+        cfg.gridDim = dim3(kNumSM / cs * cs);
+        int n = 0;
+        CU_TRY(cudaOccupancyMaxActiveClusters(&n, gemm_tf32_kernel, &cfg));
+        if (n < 1) return fail(TRIPLES_ECUDA, "no cluster of %d CTAs of the mixed contraction fits the device", cs);
+        max_clusters[cs] = std::min(n, kNumSM / cs);
+    }
+    cfg.gridDim = dim3((unsigned)(std::min<long long>(items, max_clusters[cs]) * cs));
+    if (cs == 1) {
+        gemm_tf32_kernel<<<cfg.gridDim, cfg.blockDim, cfg.dynamicSmemBytes, st>>>(maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles,
+                                                                                 P.tf_ntiles, P.tf_bn, cs, P.tf_npad, dbg);
+        CU_TRY(cudaGetLastError());
+    } else {
+        CU_TRY(cudaLaunchKernelEx(&cfg, gemm_tf32_kernel, maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles, P.tf_ntiles,
+                                  P.tf_bn, cs, P.tf_npad, dbg));
+    }
     ++g_launches;
     return TRIPLES_OK;
 }
@@ -344,32 +369,55 @@ int run_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, c
     for (const Triplet& t : trip)
         if (!(t.i == t.j && t.j == t.k)) work.push_back(t);
     const size_t nwork = work.size();
+    // batches (S1): the triplets of one block of occupied-index windows (plan.h), at most P.nb of them
+    const int win = P.win, nwin = (o + win - 1) / win;
+    auto block_key = [&](const Triplet& t) { return ((long long)(t.i / win) * nwin + t.j / win) * nwin + t.k / win; };
+    std::stable_sort(work.begin(), work.end(),
+                     [&](const Triplet& x, const Triplet& y) { return block_key(x) < block_key(y); });
+    std::vector<size_t> bstart;   // first triplet of each batch
+    for (size_t n = 0; n < nwork; ++n)
+        if (n == 0 || block_key(work[n]) != block_key(work[n - 1]) || n - bstart.back() == (size_t)P.nb) bstart.push_back(n);
+    bstart.push_back(nwork);
+    const size_t nbatch = bstart.size() - 1;
     std::vector<GemmJob> gj;
     std::vector<RedJob> rj(nwork);
     std::vector<FinJob> fj(nwork);
     std::vector<int> gj_begin;   // first gemm job of each batch
     TS* ubase = reinterpret_cast<TS*>(ws + P.off_u);
     double distinct_u = 0.0;
-    for (size_t n = 0; n < nwork; ++n) {
-        const Triplet& t = work[n];
-        const int slot = (int)(n % P.nb);
-        if (slot == 0) gj_begin.push_back((int)gj.size());
-        TS* ub = ubase + (size_t)3 * slot * P.n_u;                 // interleaved blocks of U1,U2,U3 (ulayout.cuh)
-        TS *u1 = ub, *u2 = ub + UBLK, *u3 = ub + 2 * UBLK;
-        if (t.i == t.j) {            // G(j,i,k) = G(i,j,k): one job, two destinations
-            gj.push_back({t.i, t.j, t.k, 0, u1, u2});
-            gj.push_back({t.k, t.i, t.j, 0, u3, nullptr});
-        } else if (t.j == t.k) {     // G(k,i,j) = G(j,i,k)
-            gj.push_back({t.i, t.j, t.k, 0, u1, nullptr});
-            gj.push_back({t.j, t.i, t.k, 0, u2, u3});
-        } else {
-            gj.push_back({t.i, t.j, t.k, 0, u1, nullptr});               // G(i,j,k)[a][b][c]
-            gj.push_back({t.j, t.i, t.k, 0, u2, nullptr});               // G(j,i,k)[b][a][c]
-            gj.push_back({t.k, t.i, t.j, 0, u3, nullptr});               // G(k,i,j)[c][a][b]
+    for (size_t b = 0; b < nbatch; ++b) {
+        const size_t j0 = gj.size();
+        gj_begin.push_back((int)j0);
+        for (size_t n = bstart[b]; n < bstart[b + 1]; ++n) {
+            const Triplet& t = work[n];
+            const int slot = (int)(n - bstart[b]);
+            TS* ub = ubase + (size_t)3 * slot * P.n_u;                 // interleaved blocks of U1,U2,U3 (ulayout.cuh)
+            TS *u1 = ub, *u2 = ub + UBLK, *u3 = ub + 2 * UBLK;
+            if (t.i == t.j) {            // G(j,i,k) = G(i,j,k): one job, two destinations
+                gj.push_back({t.i, t.j, t.k, 0, u1, u2, 1, {0, 0, 0}});
+                gj.push_back({t.k, t.i, t.j, 0, u3, nullptr, 1, {0, 0, 0}});
+            } else if (t.j == t.k) {     // G(k,i,j) = G(j,i,k)
+                gj.push_back({t.i, t.j, t.k, 0, u1, nullptr, 1, {0, 0, 0}});
+                gj.push_back({t.j, t.i, t.k, 0, u2, u3, 1, {0, 0, 0}});
+            } else {
+                gj.push_back({t.i, t.j, t.k, 0, u1, nullptr, 1, {0, 0, 0}});               // G(i,j,k)[a][b][c]
+                gj.push_back({t.j, t.i, t.k, 0, u2, nullptr, 1, {0, 0, 0}});               // G(j,i,k)[b][a][c]
+                gj.push_back({t.k, t.i, t.j, 0, u3, nullptr, 1, {0, 0, 0}});               // G(k,i,j)[c][a][b]
+            }
+            distinct_u += 1.0 + (t.i != t.j) + (t.j != t.k);
+            rj[n] = {t.i, t.j, t.k, slot, ub, nullptr};
+            fj[n] = {slot, (int)t.index, triplet_weight(t.i, t.j, t.k)};
         }
-        distinct_u += 1.0 + (t.i != t.j) + (t.j != t.k);
-        rj[n] = {t.i, t.j, t.k, slot, ub, nullptr};
-        fj[n] = {slot, (int)t.index, triplet_weight(t.i, t.j, t.k)};
+        // jobs with the same (q,r) read the same X_r / XT_q slices: make them neighbours and tell the kernel
+        std::sort(gj.begin() + j0, gj.end(), [](const GemmJob& x, const GemmJob& y) {
+            return x.q != y.q ? x.q < y.q : (x.r != y.r ? x.r < y.r : x.p < y.p);
+        });
+        for (size_t g = j0; g < gj.size();) {
+            size_t e = g;
+            while (e < gj.size() && gj[e].q == gj[g].q && gj[e].r == gj[g].r) ++e;
+            for (size_t x = g; x < e; ++x) { gj[x].gstart = (int)(g - j0); gj[x].gsize = (int)(e - g); }
+            g = e;
+        }
     }
     gj_begin.push_back((int)gj.size());
     GemmJob* d_gj = reinterpret_cast<GemmJob*>(ws + P.off_gjobs);
@@ -396,10 +444,9 @@ int run_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, c
 
     // ---- batches: contraction -> fused reduction -> per-triplet finalize
     std::vector<cudaEvent_t> evs;
-    const size_t nbatch = (nwork + P.nb - 1) / P.nb;
     for (size_t b = 0; b < nbatch; ++b) {
-        const size_t n0 = b * P.nb;
-        const int cnt = (int)std::min<size_t>(P.nb, nwork - n0);
+        const size_t n0 = bstart[b];
+        const int cnt = (int)(bstart[b + 1] - n0);
         const int g0 = gj_begin[b], g1 = gj_begin[b + 1];
         cudaEvent_t e[4] = {nullptr, nullptr, nullptr, nullptr};
         if (prof) {
@@ -622,7 +669,9 @@ int triples_w_block(int nocc, int nvirt, const double* t2, const double* vvvo, c
     if (int rc = build_maps(P, op, &maps)) return rc;
     uint8_t* ubase = ws + P.off_u;
     const size_t ub = (size_t)UBLK * P.esz;   // U1, U2, U3 blocks of a tile are adjacent
-    GemmJob gj[3] = {{i, j, k, 0, ubase, nullptr}, {j, i, k, 0, ubase + ub, nullptr}, {k, i, j, 0, ubase + 2 * ub, nullptr}};
+    GemmJob gj[3] = {{i, j, k, 0, ubase, nullptr, 1, {0, 0, 0}},          // three groups of one job
+                     {j, i, k, 1, ubase + ub, nullptr, 1, {0, 0, 0}},
+                     {k, i, j, 2, ubase + 2 * ub, nullptr, 1, {0, 0, 0}}};
     GemmJob* d_gj = reinterpret_cast<GemmJob*>(ws + P.off_gjobs);
     CU_TRY(cudaMemcpyAsync(d_gj, gj, sizeof gj, cudaMemcpyHostToDevice, st));
     if (int rc = launch_gemm(P, maps, d_gj, 3, st)) return rc;
