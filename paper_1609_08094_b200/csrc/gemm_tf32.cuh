@@ -58,16 +58,20 @@ constexpr int TF_CHAIN = 1;             // K chunks per TMEM accumulation chain
 constexpr int TF_TMEM_COLS = 512;
 constexpr int TF_MAX_STAGES = 4;
 constexpr int TF_SMEM_LIMIT = 227 * 1024;
+constexpr int TF_MAX_JOBS = 192;        // jobs per launch (3 per triplet, plan.h: at most 4^3 triplets per batch); the
+                                        // job table is copied to shared memory once (item -> job look-ups sit on the
+                                        // critical path of every role, two dependent global loads each otherwise)
+constexpr int TF_TAIL_BYTES = 2048 + TF_MAX_JOBS * 48;   // alignment slack + barriers, job table
 
 // npad = N-side rows a CTA stages: bn / 2 in pair mode (cs = 2), bn for a single CTA (cs = 1)
 __host__ __device__ constexpr int tf32_stage_bytes(int npad) { return 2 * TF_BM * 128 + 2 * npad * 128; }
 // stages that fit (>= 2 for every npad <= 256), capped; the dynamic smem request is always > half an SM's shared
 // memory so that exactly one CTA is resident per SM (it owns all 512 TMEM columns).
 __host__ __device__ constexpr int tf32_stages(int npad) {
-    int s = (TF_SMEM_LIMIT - 2048) / tf32_stage_bytes(npad);
+    int s = (TF_SMEM_LIMIT - TF_TAIL_BYTES) / tf32_stage_bytes(npad);
     return s > TF_MAX_STAGES ? TF_MAX_STAGES : s;
 }
-__host__ __device__ constexpr int tf32_smem_bytes(int npad) { return tf32_stages(npad) * tf32_stage_bytes(npad) + 2048; }
+__host__ __device__ constexpr int tf32_smem_bytes(int npad) { return tf32_stages(npad) * tf32_stage_bytes(npad) + TF_TAIL_BYTES; }
 
 // Work item w -> (job, tile).  The jobs of a launch are sorted by (q,r) (triples_b200.cu); the gsize jobs of a group
 // share their M-side operand slices XK_r / XKT_q / T2K_q / T2KT_r, so consecutive items are the SAME tile of the
@@ -82,7 +86,7 @@ __device__ __forceinline__ void tf32_item(const GemmJob* __restrict__ jobs, long
 }
 
 __global__ void __launch_bounds__(TF_THREADS, 1)
-gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restrict__ jobs, int njobs, int v, int vp,
+gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restrict__ gjobs, int njobs, int v, int vp,
                  int o, int mtiles, int ntiles, int bn, int cs, int npad, int dbg) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -93,6 +97,9 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
     uint64_t* tfull = empty + TF_MAX_STAGES;     // accumulator buffer ready for the epilogue
     uint64_t* tempty = tfull + 2;                // accumulator buffer drained
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+    GemmJob* jobs = reinterpret_cast<GemmJob*>(smem + stages * stage_bytes + 256);
+    for (int e = threadIdx.x; e < njobs * (int)(sizeof(GemmJob) / 4); e += TF_THREADS)
+        reinterpret_cast<uint32_t*>(jobs)[e] = reinterpret_cast<const uint32_t*>(gjobs)[e];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nrows = v * vp;                                   // flattened (b,c') rows
@@ -142,7 +149,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                     mbar_wait(&empty[s], ((it / stages) & 1) ^ 1);
                     uint8_t* sM = smem + s * stage_bytes;           // [hi 128 rows][lo 128 rows]
                     uint8_t* sN = sM + 2 * TF_BM * 128;             // [hi npad rows][lo npad rows]
-                    if (rank == 0 && !(dbg & 4)) mbar_arrive_expect_tx(&full[s], cs * stage_bytes);
+                    if (rank == 0 && !(dbg & 4)) mbar_arrive_expect_tx(&full[s], (dbg & 16) ? cs * stage_bytes / 2 : cs * stage_bytes);
                     const CUtensorMap *mm, *nm;
                     int kk, mz, nz;
                     if (c < nch_v)                     { kk = c * TF_BK;                       mm = maps.xk;   mz = r; nm = maps.t2a; nz = p * o + q; }
@@ -164,9 +171,9 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                         const int an = a0 + rank * npad;
                         if (dbg & 8) m0 = 0;
                         tma_load_3d_pair(sM, &mm[0], lbar, kk, m0, mz);
-                        tma_load_3d_pair(sM + TF_BM * 128, &mm[1], lbar, kk, m0, mz);
+                        if (!(dbg & 16)) tma_load_3d_pair(sM + TF_BM * 128, &mm[1], lbar, kk, m0, mz);
                         tma_load_3d_pair(sN, &nm[0], lbar, kk, an, nz);
-                        tma_load_3d_pair(sN + npad * 128, &nm[1], lbar, kk, an, nz);
+                        if (!(dbg & 16)) tma_load_3d_pair(sN + npad * 128, &nm[1], lbar, kk, an, nz);
                     }
                 }
             }
@@ -267,22 +274,33 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                     else mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[buf]), 0));
                 }
             }
-            // blocked + swizzled store (ulayout.cuh): this thread owns (b,c) = row, the columns are a
+            // blocked + swizzled store (ulayout.cuh): this thread owns (y,z) = (b,c) = row, the columns are x = a.
+            // The 8 a-values of a tile sit in one aligned 32-byte chunk at word (x ^ m), m = (z1 << 1) | (y0 << 2).
             const int row = m0 + wq * 32 + lane;
             const int bb = row / vp, cc = row - bb * vp;
             if (active && row < nrows && cc < v && !(dbg & 1)) {
                 float* __restrict__ out = static_cast<float*>(jobs[jb].out);
                 float* __restrict__ out2 = static_cast<float*>(jobs[jb].out2);
                 const int nt = u_tiles(v);
-                const size_t cb = ((size_t)(bb >> 3) * nt + (cc >> 3)) * UCHUNK + u_swz<4>(0, bb & 7, cc & 7);
+                const int sw = u_swz<4>(0, bb & 7, cc & 7);
+                const bool s4 = (sw & 4) != 0, s2 = (sw & 2) != 0;
                 const size_t astride = (size_t)nt * nt * UCHUNK;   // one a-tile
+                const size_t cb = (size_t)((a0 + half * 128) >> 3) * astride +
+                                  ((size_t)(bb >> 3) * nt + (cc >> 3)) * UCHUNK + (sw & ~7);
+                const int acols = min(bn, v - a0) - half * 128;    // columns of this thread that exist
 #pragma unroll
-                for (int j = 0; j < 128; ++j) {
-                    const int cl = half * 128 + j;                 // a0 is a multiple of 16: (a0 + cl) & 7 = j & 7
-                    if (cl < bn && a0 + cl < v) {
-                        const size_t off = (size_t)((a0 + cl) >> 3) * astride + (cb ^ (size_t)u_swz<4>(j & 7, 0, 0));
-                        out[off] = acc[j];
-                        if (out2) out2[off] = acc[j];
+                for (int t = 0; t < 16; ++t) {
+                    if (8 * t < acols) {
+                        float u[8], w[8];
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            u[j] = s4 ? acc[8 * t + j + 4] : acc[8 * t + j];
+                            u[j + 4] = s4 ? acc[8 * t + j] : acc[8 * t + j + 4];
+                        }
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) w[j] = s2 ? u[j ^ 2] : u[j];
+                        stg_v8(out + cb + (size_t)t * astride, w);        // one whole 32-byte sector per lane
+                        if (out2) stg_v8(out2 + cb + (size_t)t * astride, w);
                     }
                 }
             }

@@ -77,9 +77,12 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t cta_addr, uint32_t rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(cta_addr), "r"(rank));
     return r;
 }
-// arrive on an mbarrier given by its shared::cluster address (possibly in the peer CTA)
+// Arrive on an mbarrier given by its shared::cluster address (possibly in the peer CTA).  RELAXED: the arrivals of
+// the contraction kernel hand over no generic-proxy data (TMA bytes are counted by complete_tx, TMEM reads are
+// complete after tcgen05.wait::ld), and a release at cluster scope is a MEMBAR that waits for every global store the
+// thread still has in flight (ncu: 1/3 of the accumulator warps' time on this one instruction).
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster_addr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
 }
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
@@ -189,6 +192,12 @@ __device__ __forceinline__ void tmem_ld_32x32b_x16(uint32_t taddr, uint32_t (&r)
         : "memory");
 }
 // Register re-partitioning between warpgroups (all four warps of a warpgroup execute the same instruction).
+// 256-bit global store (sm_100: STG.256), 32-byte aligned
+__device__ __forceinline__ void stg_v8(float* p, const float (&w)[8]) {
+    asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(w[0]), "f"(w[1]), "f"(w[2]), "f"(w[3]),
+                 "f"(w[4]), "f"(w[5]), "f"(w[6]), "f"(w[7])
+                 : "memory");
+}
 template <int N> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }

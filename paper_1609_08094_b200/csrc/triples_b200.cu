@@ -185,6 +185,7 @@ int launch_gemm_tf32(const Tf32Maps& maps, const GemmJob* jobs, int njobs, const
         attr_set = true;
     }
     const int cs = P.tf_cs;
+    if (njobs > TF_MAX_JOBS) return fail(TRIPLES_EINVAL, "internal: %d contraction jobs in one launch (max %d)", njobs, TF_MAX_JOBS);
     const long long items = (long long)njobs * ((P.tf_mtiles + cs - 1) / cs) * P.tf_ntiles;   // per cluster
     if (items == 0) return TRIPLES_OK;
     cudaLaunchConfig_t cfg = {};

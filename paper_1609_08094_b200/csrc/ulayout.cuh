@@ -13,11 +13,15 @@
 // (a,b,c), i.e. {x0,y0,z0} plus one (two) of {x1,y1,z1} whatever the permutation:
 //
 //   FP64 (bank pair = position bits 0..3):  p = z0 | (z1^x1^y1)<<1 | (z2^x0)<<2 | y0<<3 | x0<<4 | x1<<5 | y1<<6 | x2<<7 | y2<<8
-//   FP32 (bank      = position bits 0..4):  p = z0 | (z1^y1)<<1 | (z2^x0)<<2 | y0<<3 | (x1^y1)<<4 | x0<<5 | y1<<6 | x2<<7 | y2<<8
+//   FP32 (bank      = position bits 0..4):  p = x0 | (x1^z1)<<1 | (x2^y0)<<2 | z0<<3 | (y1^z1)<<4 | y0<<5 | z1<<6 | y2<<7 | z2<<8
 //
-// The three low bits are z0, z1, z2 up to an XOR with x/y bits, so the 8 z-values of one (x,y) stay inside one aligned
-// 64-byte (FP64) / 32-byte (FP32) chunk: the GEMM epilogues write whole 32-byte sectors, and (z, z+1) pairs with z
-// even are still adjacent words.  Both maps are linear over GF(2): u_swz(x,y,z) = u_swz(x,0,0) ^ u_swz(0,y,z).
+// FP64: the three low bits are z0, z1, z2 up to an XOR with x/y bits, so the 8 z-values of one (x,y) stay inside one
+// aligned 64-byte chunk: the FP64 GEMM epilogue (a thread owns (z, z+1) column pairs) writes whole 32-byte sectors.
+// FP32: the same map with the roles rotated, S(x,y,z) = S0(y,z,x) -- the reduction reads every block in all six
+// arrangements, so any relabelling of the arguments is conflict free as well -- which puts the 8 x-values of one
+// (y,z) into one aligned 32-byte chunk: in the mixed GEMM a thread owns one (y,z) = (b,c) row and all x = a columns
+// (gemm_tf32.cuh), so its epilogue is two 16-byte stores per tile instead of eight scattered words.
+// Both maps are linear over GF(2): u_swz(x,y,z) = u_swz(x,0,0) ^ u_swz(0,y,z).
 // Elements with an index >= v inside the last tile of an axis are never written and never read.
 #pragma once
 #include <cstddef>
@@ -39,9 +43,9 @@ template <> __host__ __device__ constexpr int u_swz<8>(int x, int y, int z) {
            (((x >> 1) & 1) << 5) | (((y >> 1) & 1) << 6) | (((x >> 2) & 1) << 7) | (((y >> 2) & 1) << 8);
 }
 template <> __host__ __device__ constexpr int u_swz<4>(int x, int y, int z) {
-    return (z & 1) | ((((z ^ y) >> 1) & 1) << 1) | ((((z >> 2) ^ x) & 1) << 2) | ((y & 1) << 3) |
-           ((((x ^ y) >> 1) & 1) << 4) | ((x & 1) << 5) | (((y >> 1) & 1) << 6) | (((x >> 2) & 1) << 7) |
-           (((y >> 2) & 1) << 8);
+    return (x & 1) | ((((x ^ z) >> 1) & 1) << 1) | ((((x >> 2) ^ y) & 1) << 2) | ((z & 1) << 3) |
+           ((((y ^ z) >> 1) & 1) << 4) | ((y & 1) << 5) | (((z >> 1) & 1) << 6) | (((y >> 2) & 1) << 7) |
+           (((z >> 2) & 1) << 8);
 }
 
 // element offset of (x,y,z) of buffer u = 0 relative to the slot base (buffer u starts u * UBLK further on)
