@@ -181,7 +181,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
     } else if (warp == 1) {
         // ------------------------------------------------------------------------------------ MMA issuer
         if (lane == 0 && rank == 0) {
-            const uint32_t idesc = cs == 1 ? umma_idesc_tf32_m128((uint32_t)bn) : umma_idesc_tf32_m256((uint32_t)bn);
+            const uint32_t idesc = umma_idesc_tf32_m256((uint32_t)bn), idesc16 = umma_idesc_bf16_m256((uint32_t)bn);
             const uint32_t smem_base = smem_u32(smem);
             uint32_t it = 0, chain = 0;
             for (long long w = cid; w < nitems; w += ncl) {
@@ -207,33 +207,21 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                     const uint64_t mh = umma_desc_sw128(sM), ml = umma_desc_sw128(sM + TF_BM * 128);
                     const uint64_t nh = umma_desc_sw128(sN), nl = umma_desc_sw128(sN + npad * 128);
                     uint32_t acc = first ? 0u : 1u;
-                    if (cs == 1) {
-                        for (int k = 0; k < nk; ++k) {                   // small terms first
-                            const uint64_t adv = (uint64_t)(k * 2);      // 32 bytes per k-step, in 16-byte units
-                            umma_tf32(tacc, ml + adv, nh + adv, idesc, acc);      // lo*hi
-                            acc = 1;
-                            umma_tf32(tacc, mh + adv, nl + adv, idesc, 1);        // hi*lo
-                        }
-                        for (int k = 0; k < nk; ++k) {
-                            const uint64_t adv = (uint64_t)(k * 2);
-                            umma_tf32(tacc, mh + adv, nh + adv, idesc, 1);        // hi*hi
-                        }
-                        umma_commit(&empty[s]);       // smem slot free once these MMAs have read it
-                        if (last) { umma_commit(&tfull[buf]); ++chain; }   // chain complete
-                    } else {
-                        for (int k = 0; k < nk; ++k) {
-                            const uint64_t adv = (uint64_t)(k * 2);
-                            umma_tf32_pair(tacc, ml + adv, nh + adv, idesc, acc);
-                            acc = 1;
-                            umma_tf32_pair(tacc, mh + adv, nl + adv, idesc, 1);
-                        }
-                        for (int k = 0; k < nk; ++k) {
-                            const uint64_t adv = (uint64_t)(k * 2);
-                            umma_tf32_pair(tacc, mh + adv, nh + adv, idesc, 1);
-                        }
-                        umma_commit_pair(&empty[s]);                       // both CTAs' slots
-                        if (last) { umma_commit_pair(&tfull[buf]); ++chain; }   // both CTAs' accumulator warps
+                    // cross terms l*h' + h*l' in BF16 (packed tile: bytes 0..63 of a row = 32 BF16 of h, 64..127 = 32
+                    // BF16 of l; K = 16 per MMA), small terms first; then the main term h*h' in TF32 (K = 8 per MMA)
+                    const int nk16 = (nk + 1) >> 1;
+                    for (int k = 0; k < nk16; ++k) {
+                        const uint64_t adv = (uint64_t)(k * 2);          // 32 bytes per k-step, in 16-byte units
+                        umma_bf16_pair(tacc, ml + 4 + adv, nl + adv, idesc16, acc);   // l * h'
+                        acc = 1;
+                        umma_bf16_pair(tacc, ml + adv, nl + 4 + adv, idesc16, 1);     // h * l'
                     }
+                    for (int k = 0; k < nk; ++k) {
+                        const uint64_t adv = (uint64_t)(k * 2);
+                        umma_tf32_pair(tacc, mh + adv, nh + adv, idesc, 1);           // h * h'
+                    }
+                    umma_commit_pair(&empty[s]);                       // both CTAs' slots
+                    if (last) { umma_commit_pair(&tfull[buf]); ++chain; }   // both CTAs' accumulator warps
                 }
             }
         }

@@ -64,7 +64,7 @@ inline int tf_cluster_size() {
 
 struct Plan {
     int o = 0, v = 0, vp = 0, op = 0, prec = 0;
-    int vk = 0, ok = 0;         // mixed path: K pitches of the K-major FP32 operands (v, o rounded up to 4)
+    int vk = 0, ok = 0;         // mixed path: K pitches of the K-major FP32 operands (v, o rounded up to 32)
     int cfg = 0, BM = 0, BN = 0, mtiles = 0, ntiles = 0;      // FP64 contraction tiles
     int tf_bn = 0, tf_ntiles = 0, tf_mtiles = 0;              // mixed contraction tiles: 128 (b,c) rows x tf_bn a-columns
     int tf_cs = 1, tf_npad = 0;                               // CTAs per MMA tile (2 = cta_group::2 pair); N-side rows a CTA stages
@@ -123,8 +123,8 @@ inline bool make_plan(int o, int v, int prec, Plan& P) {
     long long ctas_per_triplet = 3LL * P.mtiles * P.ntiles;
     long long waves = 40;
     if (prec == 1) {   // K-major FP32 operands, transposed tiles (gemm_tf32.cuh)
-        P.vk = (v + 3) & ~3;
-        P.ok = (o + 3) & ~3;
+        P.vk = (v + 31) & ~31;     // whole 32-wide K chunks: the packed BF16 arrays interleave hi and lo per chunk
+        P.ok = (o + 31) & ~31;
         P.tf_ntiles = (v + 255) / 256;
         P.tf_bn = (((v + P.tf_ntiles - 1) / P.tf_ntiles) + 15) & ~15;
         P.tf_mtiles = (int)((N + 127) / 128);

@@ -7,26 +7,36 @@
 // TO is the operand type of the contraction path (double, or float for the mixed path's hi/lo split).
 #pragma once
 #include <cstdint>
+#include <cuda_bf16.h>
 
 namespace tb {
 
-// hi/lo split of a double into two floats: hi = RN_tf32-representable part, lo = remainder (also tf32-rounded).
-// Used only by the mixed path; see gemm_tf32.cuh.
+// Mixed-path split of a double x (gemm_tf32.cuh): h = RN_tf32(x) goes to the FP32 array `hi`; the second array `pk`
+// has the same geometry (rows of `pitch` floats, pitch a multiple of 32) but holds, for every chunk of 32 k, 32 BF16
+// values of h followed by 32 BF16 values of the remainder x - h: the operands of the two cross terms h*l' + l*h',
+// which only need ~9 bits (they are 2^-12 of the main term h*h').
 __device__ __forceinline__ float to_tf32_rn(float x) {
     uint32_t u;
     asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(x));
     return __uint_as_float(u);
 }
 
+__device__ __forceinline__ void put_split(float* hi, float* pk, size_t row_off, int k, double x) {
+    const float h = to_tf32_rn((float)x);
+    hi[row_off + k] = h;
+    __nv_bfloat16* p16 = reinterpret_cast<__nv_bfloat16*>(pk + row_off) + ((k >> 5) << 6) + (k & 31);
+    p16[0] = __float2bfloat16_rn(h);
+    p16[32] = __float2bfloat16_rn((float)(x - (double)h));
+}
+
+// element k of the row starting at row_off (in elements)
 template <typename TO> struct Splitter;
 template <> struct Splitter<double> {
-    static __device__ __forceinline__ void put(double* hi, double*, size_t idx, double x) { hi[idx] = x; }
+    static __device__ __forceinline__ void put(double* hi, double*, size_t row_off, int k, double x) { hi[row_off + k] = x; }
 };
 template <> struct Splitter<float> {
-    static __device__ __forceinline__ void put(float* hi, float* lo, size_t idx, double x) {
-        const float h = to_tf32_rn((float)x);
-        hi[idx] = h;
-        if (lo) lo[idx] = to_tf32_rn((float)(x - (double)h));
+    static __device__ __forceinline__ void put(float* hi, float* pk, size_t row_off, int k, double x) {
+        put_split(hi, pk, row_off, k, x);
     }
 };
 
@@ -50,7 +60,7 @@ pack_x_kernel(const double* __restrict__ vvvo, int v, int vp, int o, int RB, TO*
         const size_t Rg = R0 + rr;
         const size_t db = Rg / v;
         const int c = (int)(Rg % v);
-        Splitter<TO>::put(X, Xlo, (size_t)k * plane + db * vp + c, tile[rr * op1 + k]);
+        Splitter<TO>::put(X, Xlo, (size_t)k * plane + db * vp, c, tile[rr * op1 + k]);
     }
 }
 
@@ -80,7 +90,7 @@ __global__ void pack_ot_kernel(const double* __restrict__ ovoo, int v, int o, in
         const int p = (int)((e / ((size_t)o * v)) % o);
         const int r = (int)(e / ((size_t)o * v * o));
         const double x = -ovoo[(((size_t)p * v + a) * o + l) * o + r];
-        Splitter<TO>::put(Ot, Otlo, (((size_t)r * o + p) * v + a) * op + l, x);
+        Splitter<TO>::put(Ot, Otlo, (((size_t)r * o + p) * v + a) * op, l, x);
     }
 }
 
@@ -92,15 +102,15 @@ __global__ void pack_t2_kernel(const double* __restrict__ t2, size_t rows, int v
     for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         const size_t row = e / v;
         const int d = (int)(e % v);
-        Splitter<TO>::put(T2, T2lo, row * vp + d, t2[e]);
+        Splitter<TO>::put(T2, T2lo, row * vp, d, t2[e]);
     }
 }
 
 // ------------------------------------------------------------------------------------------------ mixed path
-// K-major FP32 operands of gemm_tf32.cuh, each as a hi/lo pair (Splitter<float>):
-//   XK  [r][b][c][d] = vvvo[d][b][c][r] = (db|cr)      (c: vp rows per b, d-pitch vk = v rounded up to 4)
+// K-major FP32 operands of gemm_tf32.cuh, each as a pair (TF32 array, packed BF16 hi|lo array; put_split):
+//   XK  [r][b][c][d] = vvvo[d][b][c][r] = (db|cr)      (c: vp rows per b, d-pitch vk = v rounded up to 32)
 //   XKT [r][b][c][d] = XK[r][c][b][d]
-//   T2K [q][b][c][l] = t2[q][l][b][c]                  (l-pitch ok = o rounded up to 4)
+//   T2K [q][b][c][l] = t2[q][l][b][c]                  (l-pitch ok = o rounded up to 32)
 //   T2KT[r][b][c][l] = t2[l][r][b][c] = t2[r][l][c][b]
 //   T2A = pack_t2_kernel with pitch vk, OtA = pack_ot_kernel with pitch ok.
 // Pads are zeroed by the caller (cudaMemsetAsync) when any exists.
@@ -132,12 +142,8 @@ pack_xk_kernel(const double* __restrict__ vvvo, int v, int vp, int vk, int o, fl
         const size_t bc = sg / o;
         const int b = (int)(bc / v), c = (int)(bc % v);
         const double x = tile[dd * PKX_PITCH + s];
-        const float h = to_tf32_rn((float)x);
-        const float l = to_tf32_rn((float)(x - (double)h));
-        const size_t i1 = (size_t)r * plane + ((size_t)b * vp + c) * vk + d0 + dd;
-        const size_t i2 = (size_t)r * plane + ((size_t)c * vp + b) * vk + d0 + dd;
-        XK[i1] = h; XKlo[i1] = l;
-        XKT[i2] = h; XKTlo[i2] = l;
+        put_split(XK, XKlo, (size_t)r * plane + ((size_t)b * vp + c) * vk, d0 + dd, x);
+        put_split(XKT, XKTlo, (size_t)r * plane + ((size_t)c * vp + b) * vk, d0 + dd, x);
     }
 }
 
@@ -158,12 +164,8 @@ pack_t2k_kernel(const double* __restrict__ t2, int v, int vp, int o, int ok, flo
     for (int e = threadIdx.x; e < nl * ny; e += 256) {
         const int l = e % nl, yy = e / nl;
         const double val = tile[l][yy];
-        const float h = to_tf32_rn((float)val);
-        const float lo = to_tf32_rn((float)(val - (double)h));
-        const size_t i1 = (((size_t)q * v + x) * vp + (y0 + yy)) * ok + l0 + l;   // T2K [q][b=x][c=y][l]
-        const size_t i2 = (((size_t)q * v + (y0 + yy)) * vp + x) * ok + l0 + l;   // T2KT[q][b=y][c=x][l] = t2[q][l][x][y]
-        T2K[i1] = h; T2Klo[i1] = lo;
-        T2KT[i2] = h; T2KTlo[i2] = lo;
+        put_split(T2K, T2Klo, (((size_t)q * v + x) * vp + (y0 + yy)) * ok, l0 + l, val);    // T2K [q][b=x][c=y][l]
+        put_split(T2KT, T2KTlo, (((size_t)q * v + (y0 + yy)) * vp + x) * ok, l0 + l, val);  // T2KT[q][b=y][c=x][l] = t2[q][l][x][y]
     }
 }
 

@@ -164,12 +164,15 @@ int build_maps_tf32(const Plan& P, const Operands& op, Tf32Maps* maps) {
     const void* ota[2] = {op.ot, op.otlo};
     int rc;
     for (int h = 0; h < 2; ++h) {
-        if ((rc = make_map3(&maps->xk[h], dt, 4, xk[h], v, NR, o, vk, NR * vk, TF_BK, TF_BM, 1))) return rc;
-        if ((rc = make_map3(&maps->xkt[h], dt, 4, xkt[h], v, NR, o, vk, NR * vk, TF_BK, TF_BM, 1))) return rc;
-        if ((rc = make_map3(&maps->t2k[h], dt, 4, t2k[h], o, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
-        if ((rc = make_map3(&maps->t2kt[h], dt, 4, t2kt[h], o, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
-        if ((rc = make_map3(&maps->t2a[h], dt, 4, t2a[h], v, v, o * o, vk, v * vk, TF_BK, P.tf_npad, 1))) return rc;
-        if ((rc = make_map3(&maps->ota[h], dt, 4, ota[h], o, v, o * o, ok, v * ok, TF_BK, P.tf_npad, 1))) return rc;
+        // h = 0: TF32 arrays, K extent = v / o (TMA zero-fills the rest of the last chunk);  h = 1: packed BF16 hi|lo
+        // arrays, whole 32-float chunks (their pads are zeroed by prepare), so the K extent is the pitch
+        const uint64_t kv = h ? vk : v, ko = h ? ok : o;
+        if ((rc = make_map3(&maps->xk[h], dt, 4, xk[h], kv, NR, o, vk, NR * vk, TF_BK, TF_BM, 1))) return rc;
+        if ((rc = make_map3(&maps->xkt[h], dt, 4, xkt[h], kv, NR, o, vk, NR * vk, TF_BK, TF_BM, 1))) return rc;
+        if ((rc = make_map3(&maps->t2k[h], dt, 4, t2k[h], ko, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
+        if ((rc = make_map3(&maps->t2kt[h], dt, 4, t2kt[h], ko, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
+        if ((rc = make_map3(&maps->t2a[h], dt, 4, t2a[h], kv, v, o * o, vk, v * vk, TF_BK, P.tf_npad, 1))) return rc;
+        if ((rc = make_map3(&maps->ota[h], dt, 4, ota[h], ko, v, o * o, ok, v * ok, TF_BK, P.tf_npad, 1))) return rc;
     }
     return TRIPLES_OK;
 }
