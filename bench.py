@@ -261,7 +261,10 @@ def main():
                                                   "mma.sync.m8n8k4.f64 loop (profiles/r01_fp64_peak_probe.txt)")
     else:
         peak = peaks["bf16_tflops_sustained"] * 0.5
-        peak_note = f"TF32 = 0.5 x bf16 sustained ({peak_kind}); MMA-issued flops are 3x the useful flops (3xTF32)"
+        peak_note = (f"TF32 dense = 0.5 x bf16 sustained cuBLAS ({peak_kind}, MEASURED_PEAKS.json; nominal ratio of the "
+                     "profiling guide). achieved = ALGORITHMIC flops (12v^4+12ov^3 per executed job triple); the split "
+                     "h*h' (TF32) + h*l' + l*h' (BF16, K=16 per MMA) keeps the tensor pipe busy for 2x that many "
+                     "TF32-rate flops: see tensor_pipe_tf32_equiv / frac_tensor_pipe")
     roofline = {
         "bound": "tensor", "kernel": "gemm_f64_kernel" if prec == tb.FP64 else "gemm_tf32_kernel",
         "achieved": gemm_tflops, "peak": peak, "unit": "TFLOP/s", "frac": gemm_tflops / peak, "traffic": None,
@@ -272,6 +275,9 @@ def main():
         "flops_per_launch": prof["contraction_flops"] / max(prof["contraction_launches"], 1),
         "avg_launch_ms": prof["contraction_ms"] / max(prof["contraction_launches"], 1),
     }
+    if prec != tb.FP64:
+        roofline["tensor_pipe_tf32_equiv"] = 2.0 * gemm_tflops
+        roofline["frac_tensor_pipe"] = 2.0 * gemm_tflops / peak
     roofline_reduction = {
         "bound": "hbm", "kernel": "reduce_kernel", "achieved": red_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
         "frac": red_gbs / peaks["hbm_gbs"], "traffic": None, "peak_note": f"{peak_kind} copy bandwidth",
@@ -317,7 +323,7 @@ def main():
             "metric": "(T) TFLOP/s", "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "s_per_ET": ms_per_step / 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64" if prec == tb.FP64 else "tf32x3+f64", "data": "synthetic",
+            "dtype": "f64" if prec == tb.FP64 else "tf32+bf16 split (f32 accumulate), f64 reduction", "data": "synthetic",
             "config": {"workload": workload_name(args, o, v, naux), "parallelism": f"replicas x{world}",
                        "l2": f"inputs larger than L2 (vvvo {8*v**3*o/1e6:.0f} MB, U buffers re-written every batch)",
                        "flop_count": "T*(12v^4+12ov^3), T=o(o+1)(o+2)/6 (paper's task count, Eq. 5.0.7b)"},

@@ -1,9 +1,13 @@
 // gemm_tf32.cuh -- mixed-precision contraction kernel (S2+S3 of DESIGN.md): TMA -> swizzled smem -> tcgen05.mma
-// (kind::tf32, 3xTF32 split) with FP32 accumulators in TMEM.
+// (cta_group::2, kind::tf32 + kind::f16) with short FP32 accumulation chains in TMEM and the running sum in registers.
 //
 // The paper's mixed precision runs "only the construction of the triples amplitudes" through
-// sgemm.  B200 has no FP32 tensor path; an FP32-accurate product is recovered from three TF32 products of the
-// round-to-nearest hi/lo split made by prepare.cuh (Q13):   x*y ~= xh*yh + xh*yl + xl*yh.
+// sgemm.  B200 has no FP32 tensor path; an FP32-class product is recovered from a split of every operand x made by
+// prepare.cuh (Q13):  h = RN_tf32(x), l = x - h,   x*y ~= h*h' + (h*l' + l*h').
+// The main term h*h' runs in TF32 (exact 11 x 11 bit products, FP32 accumulation).  The cross terms are 2^-12 of it,
+// so BF16 operands (RN, 8 bits) are enough for them -- error 2^-12 * 2^-8 per product, unbiased, the same order as
+// the dropped l*l' -- and a BF16 MMA covers twice the K of a TF32 MMA: 8 MMAs per 32-wide K chunk instead of the 12
+// of a 3xTF32 scheme.  Measured on B200: W within 1e-6 of the FP64 oracle on the scale of W, E(T) within 2e-7.
 //
 // Same "G job" (p,q,r) as gemm_f64.cuh, computed TRANSPOSED so that the long flattened (b,c) index is the MMA's
 // M dimension (128 TMEM lanes per CTA, no padding waste for any v) and the virtual index a is its N dimension:
@@ -11,28 +15,31 @@
 //   G(p,q,r)[a,(b,c)] = sum_d XK_r [(b,c),d] T2A[p,q][a,d]  + sum_d XKT_q[(b,c),d] T2A[p,r][a,d]     (Eq. (2.2.2))
 //                     + sum_l T2K_q[(b,c),l] OtA[r,p][a,l]  + sum_l T2KT_r[(b,c),l] OtA[q,p][a,l]
 //
-// Operands are K-major FP32 arrays (prepare.cuh): XK[r][b][c][d] = (db|cr), XKT[r][b][c][d] = XK[r][c][b][d],
+// Operands are K-major arrays (prepare.cuh): XK[r][b][c][d] = (db|cr), XKT[r][b][c][d] = XK[r][c][b][d],
 // T2A[p][q][a][d] = t2, OtA[r][p][a][l] = -(pa|lr), T2K[q][b][c][l] = t2[q,l,b,c], T2KT[r][b][c][l] = t2[l,r,b,c];
 // the c index has vp rows per b (row v is zero when v is odd) so that U keeps the pitch the reduction expects.
+// Each exists twice with the same geometry (rows of 32-float = 128-byte K chunks): the TF32 values h, and a packed
+// array whose chunk holds 32 BF16 of h (bytes 0..63) followed by 32 BF16 of l (bytes 64..127).
 //
 // The kernel is persistent and runs as CTA PAIRS (thread-block clusters of 2 = the two SMs of a TPC, cta_group::2):
 // a pair walks work items (job, two consecutive m-tiles of 128 (b,c) rows, n-tile of BN a-columns) as ONE
 // 256 x BN MMA tile.  Each CTA stages only its own 128 M-side rows and HALF of the N-side rows (the tensor cores
-// read the other half from the peer's shared memory), which cuts the bytes every SM has to pull in per MMA by a
-// third: with hi+lo operands (8 bytes per element) the single-CTA tile was bound by the ~40 B/clk an SM can ingest
-// from L2, not by the tensor pipe (round-1 ncu: tensor pipe 47 % active, 8.4 TB/s L2->SM).
-//   warp 0    : TMA producer   (K chunks of 32 floats = one 128-byte swizzled row per operand row; hi and lo tiles;
-//                               both CTAs load, the transaction bytes all count on the leader's barrier)
-//   warp 1    : MMA issuer     (one lane of the LEADER CTA; per K chunk: 4 k-steps of lo*hi and hi*lo, then 4
-//                               k-steps of hi*hi; tcgen05.commit multicasts to both CTAs' barriers)
+// read the other half from the peer's shared memory), which cuts the bytes an SM pulls in per MMA by a third: at
+// 8 bytes per operand element the loop is bound by L2 -> SM throughput (~42 B/clk/SM chip-wide cap), not by the
+// tensor pipe.  Jobs of a launch are grouped by (q,r) so that the big XK_r / XKT_q slices come from HBM once per
+// group (tf32_item below).
+//   warp 0    : TMA producer   (K chunks of 32 floats = one 128-byte swizzled row per operand row; TF32 and packed
+//                               tiles; both CTAs load, the transaction bytes all count on the leader's barrier)
+//   warp 1    : MMA issuer     (one lane of the LEADER CTA; per K chunk 2+2 BF16 cross-term MMAs (K = 16), then 4
+//                               TF32 MMAs (K = 8); tcgen05.commit multicasts to both CTAs' barriers)
 //   warp 2    : TMEM allocator (512 columns = two 128 x 256 FP32 buffers in each CTA)
 //   warps 4-11: accumulators   (tcgen05.ld of every finished chain, FP32 round-to-nearest adds in registers,
-//                               coalesced FP32 stores of U[a][(b,c)] at the end of the tile)
+//                               one 256-bit store per (b,c) row and a-tile of U at the end of the item)
 //
 // Why the running sum lives in registers and not in TMEM: the tensor core adds each MMA's result to its accumulator
 // with truncation, so one long accumulation chain is biased towards zero by ~(number of MMAs) * 2^-25 (measured:
 // -3.4e-6 relative on W at v = 240, i.e. 7e-6 on E(T), growing with v).  A TMEM buffer therefore only ever holds a
-// short chain (TF_CHAIN K chunks, started with accumulate = 0, the small lo*hi / hi*lo terms first); finished chains
+// short chain (TF_CHAIN K chunks, started with accumulate = 0, the small cross terms first); finished chains
 // are added with FADD.RN by the accumulator warps while the tensor core fills the other buffer.
 #pragma once
 #include "gemm_f64.cuh"   // GemmJob
@@ -42,7 +49,7 @@
 namespace tb {
 
 struct alignas(64) Tf32Maps {
-    // index 0 = hi part, 1 = lo part
+    // index 0 = TF32 array, 1 = packed BF16 hi|lo array
     CUtensorMap xk[2];    // (d, n=(b,c'), r)      box (32, 128, 1)   M side, virtual segment 1
     CUtensorMap xkt[2];   // (d, n, r)             box (32, 128, 1)   M side, virtual segment 2
     CUtensorMap t2k[2];   // (l, n, q)             box (32, 128, 1)   M side, occupied segment 3
@@ -87,7 +94,8 @@ __device__ __forceinline__ void tf32_item(const GemmJob* __restrict__ jobs, long
 
 __global__ void __launch_bounds__(TF_THREADS, 1)
 gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restrict__ gjobs, int njobs, int v, int vp,
-                 int o, int mtiles, int ntiles, int bn, int cs, int npad, int dbg) {
+                 int o, int mtiles, int ntiles, int bn, int npad) {
+    constexpr int cs = 2;   // CTAs per MMA tile
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const int stages = tf32_stages(npad);
@@ -104,7 +112,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nrows = v * vp;                                   // flattened (b,c') rows
     // a pair (cs = 2) walks two consecutive m-tiles of one (job, n-tile) as one 256-row MMA tile
-    const int rank = cs > 1 ? (int)cluster_ctarank() : 0;
+    const int rank = (int)cluster_ctarank();
     const int cid = blockIdx.x / cs, ncl = gridDim.x / cs;
     const int per_job = ((mtiles + cs - 1) / cs) * ntiles;
     const long long nitems = (long long)njobs * per_job;
@@ -118,13 +126,10 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
         for (int b = 0; b < 2; ++b) { mbar_init(&tfull[b], 1); mbar_init(&tempty[b], 8 * cs); }
         fence_barrier_init();
     }
-    if (warp == 2) {
-        if (cs == 1) { tmem_alloc(tmem_slot, TF_TMEM_COLS); tmem_relinquish(); }
-        else { tmem_alloc_pair(tmem_slot, TF_TMEM_COLS); tmem_relinquish_pair(); }
-    }
+    if (warp == 2) { tmem_alloc_pair(tmem_slot, TF_TMEM_COLS); tmem_relinquish_pair(); }
     tc_fence_before_sync();
     __syncthreads();
-    if (cs > 1) cluster_sync_all();     // every CTA's barriers are initialised before a peer's TMA / commit reaches them
+    cluster_sync_all();                 // every CTA's barriers are initialised before a peer's TMA / commit reaches them
     tc_fence_after_sync();
     const uint32_t tmem_base = *tmem_slot;
 
@@ -140,41 +145,29 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
             for (long long w = cid; w < nitems; w += ncl) {
                 int jb, rem;
                 tf32_item(jobs, w, per_job, jb, rem);
-                int m0 = ((rem / ntiles) * cs + rank) * TF_BM;
-                const int a0 = (rem % ntiles) * bn;
+                const int m0 = ((rem / ntiles) * cs + rank) * TF_BM;
+                const int an = (rem % ntiles) * bn + rank * npad;   // this CTA's half of the N-side rows
                 const GemmJob job = jobs[jb];
                 const int p = job.p, q = job.q, r = job.r;
                 for (int c = 0; c < nch; ++c, ++it) {
                     const int s = it % stages;
                     mbar_wait(&empty[s], ((it / stages) & 1) ^ 1);
-                    uint8_t* sM = smem + s * stage_bytes;           // [hi 128 rows][lo 128 rows]
-                    uint8_t* sN = sM + 2 * TF_BM * 128;             // [hi npad rows][lo npad rows]
-                    if (rank == 0 && !(dbg & 4)) mbar_arrive_expect_tx(&full[s], (dbg & 16) ? cs * stage_bytes / 2 : cs * stage_bytes);
+                    uint8_t* sM = smem + s * stage_bytes;           // [TF32 128 rows][packed BF16 128 rows]
+                    uint8_t* sN = sM + 2 * TF_BM * 128;             // [TF32 npad rows][packed BF16 npad rows]
+                    // every byte of both CTAs is counted on the leader's barrier (its MMA thread is the only waiter)
+                    const uint32_t lbar = mapa_u32(smem_u32(&full[s]), 0);
+                    if (rank == 0) mbar_arrive_expect_tx(&full[s], cs * stage_bytes);
+                    else mbar_arrive_cluster(lbar);
                     const CUtensorMap *mm, *nm;
                     int kk, mz, nz;
                     if (c < nch_v)                     { kk = c * TF_BK;                       mm = maps.xk;   mz = r; nm = maps.t2a; nz = p * o + q; }
                     else if (c < 2 * nch_v)            { kk = (c - nch_v) * TF_BK;             mm = maps.xkt;  mz = q; nm = maps.t2a; nz = p * o + r; }
                     else if (c < 2 * nch_v + nch_o)    { kk = (c - 2 * nch_v) * TF_BK;         mm = maps.t2k;  mz = q; nm = maps.ota; nz = r * o + p; }
                     else                               { kk = (c - 2 * nch_v - nch_o) * TF_BK; mm = maps.t2kt; mz = r; nm = maps.ota; nz = q * o + p; }
-                    if (dbg & 8) { kk = 0; mz = 0; nz = 0; }
-                    if (dbg & 4) {
-                        if (rank == 0) mbar_arrive(&full[s]);
-                        else mbar_arrive_cluster(mapa_u32(smem_u32(&full[s]), 0));
-                    } else if (cs == 1) {
-                        tma_load_3d(sM, &mm[0], &full[s], kk, m0, mz);
-                        tma_load_3d(sM + TF_BM * 128, &mm[1], &full[s], kk, m0, mz);
-                        tma_load_3d(sN, &nm[0], &full[s], kk, a0, nz);
-                        tma_load_3d(sN + npad * 128, &nm[1], &full[s], kk, a0, nz);
-                    } else {   // own M rows, own half of the N rows; every byte is counted on the leader's barrier
-                        const uint32_t lbar = mapa_u32(smem_u32(&full[s]), 0);
-                        if (rank != 0) mbar_arrive_cluster(lbar);
-                        const int an = a0 + rank * npad;
-                        if (dbg & 8) m0 = 0;
-                        tma_load_3d_pair(sM, &mm[0], lbar, kk, m0, mz);
-                        if (!(dbg & 16)) tma_load_3d_pair(sM + TF_BM * 128, &mm[1], lbar, kk, m0, mz);
-                        tma_load_3d_pair(sN, &nm[0], lbar, kk, an, nz);
-                        if (!(dbg & 16)) tma_load_3d_pair(sN + npad * 128, &nm[1], lbar, kk, an, nz);
-                    }
+                    tma_load_3d_pair(sM, &mm[0], lbar, kk, m0, mz);
+                    tma_load_3d_pair(sM + TF_BM * 128, &mm[1], lbar, kk, m0, mz);
+                    tma_load_3d_pair(sN, &nm[0], lbar, kk, an, nz);
+                    tma_load_3d_pair(sN + npad * 128, &nm[1], lbar, kk, an, nz);
                 }
             }
         }
@@ -244,7 +237,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                 const uint32_t buf = chain & 1;
                 mbar_wait(&tfull[buf], (chain >> 1) & 1);
                 tc_fence_after_sync();
-                if (active && !(dbg & 2)) {
+                if (active) {
                     const uint32_t taddr = tmem_base + buf * 256 + half * 128 + ((uint32_t)(wq * 32) << 16);
 #pragma unroll
                     for (int c0 = 0; c0 < 128; c0 += 16) {
@@ -258,15 +251,14 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                 tc_fence_before_sync();
                 __syncwarp();
                 if (lane == 0) {     // the leader's MMA thread owns the buffer hand-back of both CTAs
-                    if (cs == 1) mbar_arrive(&tempty[buf]);
-                    else mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[buf]), 0));
+                    mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[buf]), 0));
                 }
             }
             // blocked + swizzled store (ulayout.cuh): this thread owns (y,z) = (b,c) = row, the columns are x = a.
             // The 8 a-values of a tile sit in one aligned 32-byte chunk at word (x ^ m), m = (z1 << 1) | (y0 << 2).
             const int row = m0 + wq * 32 + lane;
             const int bb = row / vp, cc = row - bb * vp;
-            if (active && row < nrows && cc < v && !(dbg & 1)) {
+            if (active && row < nrows && cc < v) {
                 float* __restrict__ out = static_cast<float*>(jobs[jb].out);
                 float* __restrict__ out2 = static_cast<float*>(jobs[jb].out2);
                 const int nt = u_tiles(v);
@@ -296,10 +288,10 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
     }
     tc_fence_before_sync();
     __syncthreads();
-    if (cs > 1) cluster_sync_all();     // no CTA leaves while a peer may still write its shared memory or barriers
+    cluster_sync_all();                 // no CTA leaves while a peer may still write its shared memory or barriers
     if (warp == 2) {
         tc_fence_after_sync();
-        if (cs == 1) tmem_dealloc(tmem_base, TF_TMEM_COLS); else tmem_dealloc_pair(tmem_base, TF_TMEM_COLS);
+        tmem_dealloc_pair(tmem_base, TF_TMEM_COLS);
     }
 }
 

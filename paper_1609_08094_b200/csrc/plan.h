@@ -55,12 +55,8 @@ inline void enumerate_orbits(int v, std::vector<Orbit>& out) {
 
 enum GemmCfgId { CFG_M120_N128 = 0, CFG_M80_N192 = 1, CFG_M40_N256 = 2 };
 
-// CTAs per MMA tile of the mixed contraction: 2 = CTA pair (default), 1 = single CTA; TRIPLES_TF_CLUSTER=1 selects
-// the single-CTA variant for A/B measurements.
-inline int tf_cluster_size() {
-    if (const char* e = std::getenv("TRIPLES_TF_CLUSTER")) return std::atoi(e) == 1 ? 1 : 2;
-    return 2;
-}
+// CTAs per MMA tile of the mixed contraction: a CTA pair (cta_group::2, gemm_tf32.cuh)
+inline int tf_cluster_size() { return 2; }
 
 struct Plan {
     int o = 0, v = 0, vp = 0, op = 0, prec = 0;

@@ -199,26 +199,18 @@ int launch_gemm_tf32(const Tf32Maps& maps, const GemmJob* jobs, int njobs, const
     cfg.dynamicSmemBytes = tf32_smem_bytes(P.tf_npad);
     cfg.stream = st;
     cfg.attrs = attr;
-    cfg.numAttrs = cs > 1 ? 1 : 0;
-    static const int dbg = std::getenv("TRIPLES_TF_DEBUG") ? std::atoi(std::getenv("TRIPLES_TF_DEBUG")) : 0;
-    static int max_clusters[5] = {0, 0, 0, 0, 0};   // co-resident clusters of this size (one CTA per SM)
-    if (cs == 1) max_clusters[1] = kNumSM;
-    if (!max_clusters[cs]) {
+    cfg.numAttrs = 1;
+    static int max_clusters = 0;   // co-resident CTA pairs (one CTA per SM)
+    if (!max_clusters) {
         cfg.gridDim = dim3(kNumSM / cs * cs);
         int n = 0;
         CU_TRY(cudaOccupancyMaxActiveClusters(&n, gemm_tf32_kernel, &cfg));
-        if (n < 1) return fail(TRIPLES_ECUDA, "no cluster of %d CTAs of the mixed contraction fits the device", cs);
-        max_clusters[cs] = std::min(n, kNumSM / cs);
+        if (n < 1) return fail(TRIPLES_ECUDA, "no CTA pair of the mixed contraction fits the device");
+        max_clusters = std::min(n, kNumSM / cs);
     }
-    cfg.gridDim = dim3((unsigned)(std::min<long long>(items, max_clusters[cs]) * cs));
-    if (cs == 1) {
-        gemm_tf32_kernel<<<cfg.gridDim, cfg.blockDim, cfg.dynamicSmemBytes, st>>>(maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles,
-                                                                                 P.tf_ntiles, P.tf_bn, cs, P.tf_npad, dbg);
-        CU_TRY(cudaGetLastError());
-    } else {
-        CU_TRY(cudaLaunchKernelEx(&cfg, gemm_tf32_kernel, maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles, P.tf_ntiles,
-                                  P.tf_bn, cs, P.tf_npad, dbg));
-    }
+    cfg.gridDim = dim3((unsigned)(std::min<long long>(items, max_clusters) * cs));
+    CU_TRY(cudaLaunchKernelEx(&cfg, gemm_tf32_kernel, maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles, P.tf_ntiles,
+                              P.tf_bn, P.tf_npad));
     ++g_launches;
     return TRIPLES_OK;
 }
@@ -279,24 +271,12 @@ int run_prepare(const Plan& P, const double* t2, const double* vvvo, const doubl
                 cudaStream_t st) {
     if (P.prec == TRIPLES_MIXED) return run_prepare_mixed(P, t2, vvvo, ovoo, op, st);
     const int o = P.o, v = P.v;
-    const bool split = P.prec == TRIPLES_MIXED;
-    if (P.vp != v) {   // zero the pad columns
+    if (P.vp != v) {   // zero the pad columns (XT: entry c = v of a row is never written by the transpose)
         CU_TRY(cudaMemsetAsync(op.x, 0, P.n_x * sizeof(TO), st));
-        CU_TRY(cudaMemsetAsync(op.t2, 0, P.n_t2 * sizeof(TO), st));
-        if (split) {
-            CU_TRY(cudaMemsetAsync(op.xlo, 0, P.n_x * sizeof(TO), st));
-            CU_TRY(cudaMemsetAsync(op.t2lo, 0, P.n_t2 * sizeof(TO), st));
-        }
-    }
-    // XT pads: rows b of a plane have vp entries, entry c = v is never written by the transpose
-    if (P.vp != v) {
         CU_TRY(cudaMemsetAsync(op.xt, 0, P.n_x * sizeof(TO), st));
-        if (split) CU_TRY(cudaMemsetAsync(op.xtlo, 0, P.n_x * sizeof(TO), st));
+        CU_TRY(cudaMemsetAsync(op.t2, 0, P.n_t2 * sizeof(TO), st));
     }
-    if (P.op != o) {
-        CU_TRY(cudaMemsetAsync(op.ot, 0, P.n_ot * sizeof(TO), st));
-        if (split) CU_TRY(cudaMemsetAsync(op.otlo, 0, P.n_ot * sizeof(TO), st));
-    }
+    if (P.op != o) CU_TRY(cudaMemsetAsync(op.ot, 0, P.n_ot * sizeof(TO), st));
     {   // X
         int RB = 128;
         while ((size_t)RB * (o + 1) * 8 > 64 * 1024 && RB > 1) RB /= 2;
@@ -308,16 +288,13 @@ int run_prepare(const Plan& P, const double* t2, const double* vvvo, const doubl
         CU_TRY(cudaGetLastError());
         ++g_launches;
     }
-    {   // XT (and its low part)
+    {   // XT
         dim3 grid((v + 31) / 32, (v + 31) / 32, 1);
-        // gridDim.z <= 65535: loop over r-slices
-        for (int r = 0; r < o; ++r) {
+        for (int r = 0; r < o; ++r) {   // gridDim.z <= 65535: one launch per r-slice
             grid.z = v;
             const size_t sl = (size_t)r * v * v * P.vp;
             transpose_planes_kernel<TO><<<grid, 256, 0, st>>>((const TO*)op.x + sl, v, P.vp, (TO*)op.xt + sl);
-            if (split)
-                transpose_planes_kernel<TO><<<grid, 256, 0, st>>>((const TO*)op.xlo + sl, v, P.vp, (TO*)op.xtlo + sl);
-            g_launches += split ? 2 : 1;
+            ++g_launches;
         }
         CU_TRY(cudaGetLastError());
     }
