@@ -49,36 +49,35 @@
 namespace tb {
 
 struct alignas(64) Tf32Maps {
-    // index 0 = TF32 array, 1 = packed BF16 hi|lo array
-    CUtensorMap xk[2];    // (d, n=(b,c'), r)      box (32, 128, 1)   M side, virtual segment 1
-    CUtensorMap xkt[2];   // (d, n, r)             box (32, 128, 1)   M side, virtual segment 2
-    CUtensorMap t2k[2];   // (l, n, q)             box (32, 128, 1)   M side, occupied segment 3
-    CUtensorMap t2kt[2];  // (l, n, r)             box (32, 128, 1)   M side, occupied segment 4
-    CUtensorMap t2a[2];   // (d, a, p*o+q)         box (32, BN, 1)    N side, virtual segments
-    CUtensorMap ota[2];   // (l, a, r*o+p)         box (32, BN, 1)    N side, occupied segments
+    CUtensorMap xk;    // (d, n=(b,c'), r)      box (32, 128, 1)    M side, virtual segment 1
+    CUtensorMap xkt;   // (d, n, r)             box (32, 128, 1)    M side, virtual segment 2
+    CUtensorMap t2k;   // (l, n, q)             box (32, 128, 1)    M side, occupied segment 3
+    CUtensorMap t2kt;  // (l, n, r)             box (32, 128, 1)    M side, occupied segment 4
+    CUtensorMap t2a;   // (d, a, p*o+q)         box (32, BN/2, 1)   N side, virtual segments
+    CUtensorMap ota;   // (l, a, r*o+p)         box (32, BN/2, 1)   N side, occupied segments
 };
 
 constexpr int TF_BM = 128;            // (b,c) rows per CTA tile = TMEM lanes
 constexpr int TF_BK = 32;             // floats per K chunk (128-byte rows)
-constexpr int TF_THREADS = 384;         // 4 service warps + 8 accumulator warps
+constexpr int TF_THREADS = 512;         // 8 service warps (TMA, MMA, TMEM, 4 converters) + 8 accumulator warps
+constexpr int TF_CONV_WARPS = 6;        // warps 2..7
 constexpr int TF_CHAIN = 1;             // K chunks per TMEM accumulation chain
 constexpr int TF_TMEM_COLS = 512;
-constexpr int TF_MAX_STAGES = 4;
 constexpr int TF_SMEM_LIMIT = 227 * 1024;
 constexpr int TF_MAX_JOBS = 192;        // jobs per launch (3 per triplet, plan.h: at most 4^3 triplets per batch); the
                                         // job table is copied to shared memory once (item -> job look-ups sit on the
                                         // critical path of every role, two dependent global loads each otherwise)
 constexpr int TF_TAIL_BYTES = 2048 + TF_MAX_JOBS * 48;   // alignment slack + barriers, job table
 
-// npad = N-side rows a CTA stages: bn / 2 in pair mode (cs = 2), bn for a single CTA (cs = 1)
-__host__ __device__ constexpr int tf32_stage_bytes(int npad) { return 2 * TF_BM * 128 + 2 * npad * 128; }
-// stages that fit (>= 2 for every npad <= 256), capped; the dynamic smem request is always > half an SM's shared
-// memory so that exactly one CTA is resident per SM (it owns all 512 TMEM columns).
-__host__ __device__ constexpr int tf32_stages(int npad) {
-    int s = (TF_SMEM_LIMIT - TF_TAIL_BYTES) / tf32_stage_bytes(npad);
-    return s > TF_MAX_STAGES ? TF_MAX_STAGES : s;
+// npad = N-side rows a CTA stages = bn / 2.  Two shared-memory rings of (128 + npad)-row tiles with 128-byte rows:
+// TF_RAW_STAGES raw tiles (TMA destination, TF32 operand; deep enough to cover the L2/HBM latency) and TF_PK_STAGES
+// packed BF16 tiles (written by the converter warps; the conversion of chunk c+1 overlaps the MMAs of chunk c).
+constexpr int TF_RAW_STAGES = 4, TF_PK_STAGES = 2;
+__host__ __device__ constexpr int tf32_tile_bytes(int npad) { return (TF_BM + npad) * 128; }
+// the request is always > half an SM's shared memory: exactly one CTA per SM (it owns all 512 TMEM columns)
+__host__ __device__ constexpr int tf32_smem_bytes(int npad) {
+    return (TF_RAW_STAGES + TF_PK_STAGES) * tf32_tile_bytes(npad) + TF_TAIL_BYTES;
 }
-__host__ __device__ constexpr int tf32_smem_bytes(int npad) { return tf32_stages(npad) * tf32_stage_bytes(npad) + TF_TAIL_BYTES; }
 
 // Work item w -> (job, tile).  The jobs of a launch are sorted by (q,r) (triples_b200.cu); the gsize jobs of a group
 // share their M-side operand slices XK_r / XKT_q / T2K_q / T2KT_r, so consecutive items are the SAME tile of the
@@ -98,14 +97,18 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
     constexpr int cs = 2;   // CTAs per MMA tile
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    const int stages = tf32_stages(npad);
-    const int stage_bytes = tf32_stage_bytes(npad);
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem + stages * stage_bytes);
-    uint64_t* empty = full + TF_MAX_STAGES;
-    uint64_t* tfull = empty + TF_MAX_STAGES;     // accumulator buffer ready for the epilogue
+    constexpr int RS = TF_RAW_STAGES, PS = TF_PK_STAGES;
+    const int tile_bytes = tf32_tile_bytes(npad);
+    uint8_t* smem_pk = smem + RS * tile_bytes;
+    uint8_t* smem_tail = smem_pk + PS * tile_bytes;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_tail);   // [RS] raw tile landed (per CTA)
+    uint64_t* empty = full + RS;                 // [RS] raw tile consumed by the MMAs
+    uint64_t* conv = empty + RS;                 // [PS] packed tile written by both CTAs' converters (leader's is used)
+    uint64_t* pkempty = conv + PS;               // [PS] packed tile consumed by the MMAs
+    uint64_t* tfull = pkempty + PS;              // accumulator buffer ready for the epilogue
     uint64_t* tempty = tfull + 2;                // accumulator buffer drained
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
-    GemmJob* jobs = reinterpret_cast<GemmJob*>(smem + stages * stage_bytes + 256);
+    GemmJob* jobs = reinterpret_cast<GemmJob*>(smem_tail + 256);
     for (int e = threadIdx.x; e < njobs * (int)(sizeof(GemmJob) / 4); e += TF_THREADS)
         reinterpret_cast<uint32_t*>(jobs)[e] = reinterpret_cast<const uint32_t*>(gjobs)[e];
 
@@ -121,8 +124,9 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
     const int nch = 2 * (nch_v + nch_o);
 
     if (threadIdx.x == 0) {
-        // full / tempty are waited on by the leader's MMA thread only: both CTAs' producers (accumulator warps) arrive
-        for (int s = 0; s < stages; ++s) { mbar_init(&full[s], cs); mbar_init(&empty[s], 1); }
+        // conv / tempty are waited on by the leader's MMA thread only: both CTAs' converter / accumulator warps arrive
+        for (int s = 0; s < RS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < PS; ++s) { mbar_init(&conv[s], TF_CONV_WARPS * cs); mbar_init(&pkempty[s], 1); }
         for (int b = 0; b < 2; ++b) { mbar_init(&tfull[b], 1); mbar_init(&tempty[b], 8 * cs); }
         fence_barrier_init();
     }
@@ -133,14 +137,12 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
     tc_fence_after_sync();
     const uint32_t tmem_base = *tmem_slot;
 
-    if (warp < 4) reg_dealloc<72>();
+    if (warp < 8) reg_dealloc<48>();
     if (warp == 0) {
         // ------------------------------------------------------------------------------------ TMA producer
         if (lane == 0) {
-            for (int h = 0; h < 2; ++h) {
-                tma_prefetch_desc(&maps.xk[h]); tma_prefetch_desc(&maps.xkt[h]); tma_prefetch_desc(&maps.t2k[h]);
-                tma_prefetch_desc(&maps.t2kt[h]); tma_prefetch_desc(&maps.t2a[h]); tma_prefetch_desc(&maps.ota[h]);
-            }
+            tma_prefetch_desc(&maps.xk); tma_prefetch_desc(&maps.xkt); tma_prefetch_desc(&maps.t2k);
+            tma_prefetch_desc(&maps.t2kt); tma_prefetch_desc(&maps.t2a); tma_prefetch_desc(&maps.ota);
             uint32_t it = 0;
             for (long long w = cid; w < nitems; w += ncl) {
                 int jb, rem;
@@ -150,25 +152,60 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                 const GemmJob job = jobs[jb];
                 const int p = job.p, q = job.q, r = job.r;
                 for (int c = 0; c < nch; ++c, ++it) {
-                    const int s = it % stages;
-                    mbar_wait(&empty[s], ((it / stages) & 1) ^ 1);
-                    uint8_t* sM = smem + s * stage_bytes;           // [TF32 128 rows][packed BF16 128 rows]
-                    uint8_t* sN = sM + 2 * TF_BM * 128;             // [TF32 npad rows][packed BF16 npad rows]
-                    // every byte of both CTAs is counted on the leader's barrier (its MMA thread is the only waiter)
-                    const uint32_t lbar = mapa_u32(smem_u32(&full[s]), 0);
-                    if (rank == 0) mbar_arrive_expect_tx(&full[s], cs * stage_bytes);
-                    else mbar_arrive_cluster(lbar);
+                    const int s = it % RS;
+                    mbar_wait(&empty[s], ((it / RS) & 1) ^ 1);
+                    uint8_t* sM = smem + s * tile_bytes;            // raw FP32 words: [M 128 rows][N npad rows]
+                    uint8_t* sN = sM + TF_BM * 128;
+                    mbar_arrive_expect_tx(&full[s], (TF_BM + npad) * 128);
                     const CUtensorMap *mm, *nm;
                     int kk, mz, nz;
-                    if (c < nch_v)                     { kk = c * TF_BK;                       mm = maps.xk;   mz = r; nm = maps.t2a; nz = p * o + q; }
-                    else if (c < 2 * nch_v)            { kk = (c - nch_v) * TF_BK;             mm = maps.xkt;  mz = q; nm = maps.t2a; nz = p * o + r; }
-                    else if (c < 2 * nch_v + nch_o)    { kk = (c - 2 * nch_v) * TF_BK;         mm = maps.t2k;  mz = q; nm = maps.ota; nz = r * o + p; }
-                    else                               { kk = (c - 2 * nch_v - nch_o) * TF_BK; mm = maps.t2kt; mz = r; nm = maps.ota; nz = q * o + p; }
-                    tma_load_3d_pair(sM, &mm[0], lbar, kk, m0, mz);
-                    tma_load_3d_pair(sM + TF_BM * 128, &mm[1], lbar, kk, m0, mz);
-                    tma_load_3d_pair(sN, &nm[0], lbar, kk, an, nz);
-                    tma_load_3d_pair(sN + npad * 128, &nm[1], lbar, kk, an, nz);
+                    if (c < nch_v)                     { kk = c * TF_BK;                       mm = &maps.xk;   mz = r; nm = &maps.t2a; nz = p * o + q; }
+                    else if (c < 2 * nch_v)            { kk = (c - nch_v) * TF_BK;             mm = &maps.xkt;  mz = q; nm = &maps.t2a; nz = p * o + r; }
+                    else if (c < 2 * nch_v + nch_o)    { kk = (c - 2 * nch_v) * TF_BK;         mm = &maps.t2k;  mz = q; nm = &maps.ota; nz = r * o + p; }
+                    else                               { kk = (c - 2 * nch_v - nch_o) * TF_BK; mm = &maps.t2kt; mz = r; nm = &maps.ota; nz = q * o + p; }
+                    tma_load_3d(sM, mm, &full[s], kk, m0, mz);
+                    tma_load_3d(sN, nm, &full[s], kk, an, nz);
                 }
+            }
+        }
+    } else if (warp >= 2 && warp < 8) {
+        // ------------------------------------------------------------------------------------ converters
+        // Operand split inside the SM (Q13): the staged word is the FP32 bit pattern of x plus 0x1000, which
+        // the TF32 MMA reads as h = RN_tf32(x) (it ignores the low 13 bits).  These warps turn every 8 consecutive k of
+        // a row into 8 BF16 of h (packed bytes 0..63 of the row) and 8 BF16 of l = x - h (bytes 64..127), honouring the
+        // 128-byte swizzle of both tiles (16-byte unit u of row R sits at unit u ^ (R & 7)).
+        const int ct = threadIdx.x - 64;
+        const int rows = TF_BM + npad;
+        const uint32_t smem_base = smem_u32(smem);
+        const uint32_t lconv0 = mapa_u32(smem_u32(&conv[0]), 0);
+        uint32_t it = 0;
+        for (long long w = cid; w < nitems; w += ncl) {
+            for (int c = 0; c < nch; ++c, ++it) {
+                const int s = it % RS, ps = it % PS;
+                mbar_wait(&pkempty[ps], ((it / PS) & 1) ^ 1);
+                mbar_wait(&full[s], (it / RS) & 1);
+                const uint32_t raw = smem_base + s * tile_bytes, pk = smem_base + (RS + ps) * tile_bytes;
+                for (int task = ct; task < rows * 4; task += 32 * TF_CONV_WARPS) {
+                    const int m = (task >> 3) & 3, R = (task & 7) | ((task >> 5) << 3);   // 8 lanes: one m, 8 rows
+                    const uint32_t rb = (uint32_t)R * 128u, sw = (uint32_t)(R & 7);
+                    uint32_t x[8];
+                    lds_v4(raw + rb + (((2 * m) ^ sw) << 4), x[0], x[1], x[2], x[3]);
+                    lds_v4(raw + rb + (((2 * m + 1) ^ sw) << 4), x[4], x[5], x[6], x[7]);
+                    float h[8], l[8];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        // a zero word (TMA zero fill, pads) stands for x = 0: max() keeps the subtraction from wrapping
+                        h[j] = __uint_as_float(x[j] & 0xffffe000u);
+                        l[j] = __uint_as_float(max(x[j], 0x1000u) - 0x1000u) - h[j];
+                    }
+                    sts_v4(pk + rb + (((uint32_t)m ^ sw) << 4), pack_bf16x2(h[0], h[1]), pack_bf16x2(h[2], h[3]),
+                           pack_bf16x2(h[4], h[5]), pack_bf16x2(h[6], h[7]));
+                    sts_v4(pk + rb + (((uint32_t)(4 + m) ^ sw) << 4), pack_bf16x2(l[0], l[1]), pack_bf16x2(l[2], l[3]),
+                           pack_bf16x2(l[4], l[5]), pack_bf16x2(l[6], l[7]));
+                }
+                fence_proxy_async();          // generic-proxy writes -> visible to the tensor core's (async proxy) reads
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster_release(lconv0 + 8u * ps);
             }
         }
     } else if (warp == 1) {
@@ -179,7 +216,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
             uint32_t it = 0, chain = 0;
             for (long long w = cid; w < nitems; w += ncl) {
                 for (int c = 0; c < nch; ++c, ++it) {
-                    const int s = it % stages;
+                    const int s = it % RS, ps = it % PS;
                     int left;   // k-steps of this chunk that carry data
                     if (c < nch_v) left = kst_v - c * 4;
                     else if (c < 2 * nch_v) left = kst_v - (c - nch_v) * 4;
@@ -192,13 +229,13 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                         mbar_wait(&tempty[buf], ((chain >> 1) & 1) ^ 1);
                         tc_fence_after_sync();
                     }
-                    mbar_wait(&full[s], (it / stages) & 1);
+                    mbar_wait(&conv[ps], (it / PS) & 1);
                     tc_fence_after_sync();
                     const uint32_t tacc = tmem_base + buf * 256;
-                    const uint32_t sM = smem_base + s * stage_bytes;
-                    const uint32_t sN = sM + 2 * TF_BM * 128;
-                    const uint64_t mh = umma_desc_sw128(sM), ml = umma_desc_sw128(sM + TF_BM * 128);
-                    const uint64_t nh = umma_desc_sw128(sN), nl = umma_desc_sw128(sN + npad * 128);
+                    const uint32_t sM = smem_base + s * tile_bytes, sN = sM + TF_BM * 128;              // raw (TF32)
+                    const uint32_t pM = smem_base + (RS + ps) * tile_bytes, pN = pM + TF_BM * 128;      // packed
+                    const uint64_t mh = umma_desc_sw128(sM), ml = umma_desc_sw128(pM);
+                    const uint64_t nh = umma_desc_sw128(sN), nl = umma_desc_sw128(pN);
                     uint32_t acc = first ? 0u : 1u;
                     // cross terms l*h' + h*l' in BF16 (packed tile: bytes 0..63 of a row = 32 BF16 of h, 64..127 = 32
                     // BF16 of l; K = 16 per MMA), small terms first; then the main term h*h' in TF32 (K = 8 per MMA)
@@ -213,16 +250,17 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                         const uint64_t adv = (uint64_t)(k * 2);
                         umma_tf32_pair(tacc, mh + adv, nh + adv, idesc, 1);           // h * h'
                     }
-                    umma_commit_pair(&empty[s]);                       // both CTAs' slots
+                    umma_commit_pair(&empty[s]);                       // both CTAs' raw and packed slots
+                    umma_commit_pair(&pkempty[ps]);
                     if (last) { umma_commit_pair(&tfull[buf]); ++chain; }   // both CTAs' accumulator warps
                 }
             }
         }
-    } else if (warp >= 4) {
+    } else if (warp >= 8) {
         // ------------------------------------------------------------------------------------ accumulator warps
-        reg_alloc<208>();   // 128*72 + 256*208 <= 64K registers
+        reg_alloc<208>();   // 256*48 + 256*208 = 64K registers
         const int wq = warp & 3;                 // TMEM lane quarter this warp may read
-        const int half = (warp - 4) >> 2;        // columns [128*half, 128*half + 128)
+        const int half = (warp - 8) >> 2;        // columns [128*half, 128*half + 128)
         const int nchain = (nch + TF_CHAIN - 1) / TF_CHAIN;
         const bool active = half * 128 < bn;
         uint32_t chain = 0;

@@ -60,7 +60,7 @@ inline int tf_cluster_size() { return 2; }
 
 struct Plan {
     int o = 0, v = 0, vp = 0, op = 0, prec = 0;
-    int vk = 0, ok = 0;         // mixed path: K pitches of the K-major FP32 operands (v, o rounded up to 32)
+    int vk = 0, ok = 0;         // mixed path: K pitches of the K-major FP32 operands (v, o rounded up to 4)
     int cfg = 0, BM = 0, BN = 0, mtiles = 0, ntiles = 0;      // FP64 contraction tiles
     int tf_bn = 0, tf_ntiles = 0, tf_mtiles = 0;              // mixed contraction tiles: 128 (b,c) rows x tf_bn a-columns
     int tf_cs = 1, tf_npad = 0;                               // CTAs per MMA tile (2 = cta_group::2 pair); N-side rows a CTA stages
@@ -74,9 +74,9 @@ struct Plan {
     size_t esz = 8;             // bytes per stored operand / U element
     size_t n_x = 0, n_ot = 0, n_t2 = 0, n_u = 0;   // elements of one X (or XT), Ot, T2, one U buffer
     size_t n_t2k = 0;                              // mixed: elements of T2K (or T2KT)
-    size_t off_t2k = 0, off_t2kt = 0, off_t2klo = 0, off_t2ktlo = 0;
+    size_t off_t2k = 0, off_t2kt = 0;
     // workspace offsets (bytes)
-    size_t off_x = 0, off_xt = 0, off_ot = 0, off_t2 = 0, off_xlo = 0, off_xtlo = 0, off_otlo = 0, off_t2lo = 0;
+    size_t off_x = 0, off_xt = 0, off_ot = 0, off_t2 = 0;
     size_t off_u = 0, off_part = 0, off_etrip = 0, off_result = 0, off_gjobs = 0, off_rjobs = 0, off_fjobs = 0,
            off_orb = 0;
     size_t total = 0;
@@ -119,8 +119,8 @@ inline bool make_plan(int o, int v, int prec, Plan& P) {
     long long ctas_per_triplet = 3LL * P.mtiles * P.ntiles;
     long long waves = 40;
     if (prec == 1) {   // K-major FP32 operands, transposed tiles (gemm_tf32.cuh)
-        P.vk = (v + 31) & ~31;     // whole 32-wide K chunks: the packed BF16 arrays interleave hi and lo per chunk
-        P.ok = (o + 31) & ~31;
+        P.vk = (v + 3) & ~3;       // 16-byte row pitch for TMA
+        P.ok = (o + 3) & ~3;
         P.tf_ntiles = (v + 255) / 256;
         P.tf_bn = (((v + P.tf_ntiles - 1) / P.tf_ntiles) + 15) & ~15;
         P.tf_mtiles = (int)((N + 127) / 128);
@@ -155,15 +155,9 @@ inline bool make_plan(int o, int v, int prec, Plan& P) {
     P.off_xt = take(P.n_x * P.esz);
     P.off_ot = take(P.n_ot * P.esz);
     P.off_t2 = take(P.n_t2 * P.esz);
-    if (prec == 1) {   // low parts of the hi/lo split
-        P.off_xlo = take(P.n_x * P.esz);
-        P.off_xtlo = take(P.n_x * P.esz);
-        P.off_otlo = take(P.n_ot * P.esz);
-        P.off_t2lo = take(P.n_t2 * P.esz);
+    if (prec == 1) {   // occupied-segment M-side operands of the transposed mixed GEMM
         P.off_t2k = take(P.n_t2k * P.esz);
         P.off_t2kt = take(P.n_t2k * P.esz);
-        P.off_t2klo = take(P.n_t2k * P.esz);
-        P.off_t2ktlo = take(P.n_t2k * P.esz);
     }
     P.off_u = take((size_t)P.nb * 3 * P.n_u * P.esz);
     P.red_gx = P.norb < kNumSM ? P.norb : kNumSM;

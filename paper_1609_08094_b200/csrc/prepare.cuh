@@ -4,30 +4,16 @@
 //   XT[r][d][b][c] = X[r][d][c][b]
 //   Ot[r][p][a][l] = -ovoo[p][a][l][r] = -(pa|lr)      (l-pitch op = o rounded up to even, pad zeroed)
 //   T2[p][q][a][d] = t2[p][q][a][d]                    (d-pitch vp, pad zeroed)
-// TO is the operand type of the contraction path (double, or float for the mixed path's hi/lo split).
+// TO is the operand type of the contraction path (double; float = the mixed path's biased FP32 words).
 #pragma once
 #include <cstdint>
-#include <cuda_bf16.h>
 
 namespace tb {
 
-// Mixed-path split of a double x (gemm_tf32.cuh): h = RN_tf32(x) goes to the FP32 array `hi`; the second array `pk`
-// has the same geometry (rows of `pitch` floats, pitch a multiple of 32) but holds, for every chunk of 32 k, 32 BF16
-// values of h followed by 32 BF16 values of the remainder x - h: the operands of the two cross terms h*l' + l*h',
-// which only need ~9 bits (they are 2^-12 of the main term h*h').
-__device__ __forceinline__ float to_tf32_rn(float x) {
-    uint32_t u;
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(x));
-    return __uint_as_float(u);
-}
-
-__device__ __forceinline__ void put_split(float* hi, float* pk, size_t row_off, int k, double x) {
-    const float h = to_tf32_rn((float)x);
-    hi[row_off + k] = h;
-    __nv_bfloat16* p16 = reinterpret_cast<__nv_bfloat16*>(pk + row_off) + ((k >> 5) << 6) + (k & 31);
-    p16[0] = __float2bfloat16_rn(h);
-    p16[32] = __float2bfloat16_rn((float)(x - (double)h));
-}
+// Mixed-path operand word (gemm_tf32.cuh): the FP32 bit pattern of RN_fp32(x) plus 0x1000 (half a TF32 ulp, added to
+// the magnitude).  A TF32 MMA ignores the low 13 bits, so it reads this word as h = RN_tf32(x) (round half away, what
+// cvt.rna.tf32.f32 gives); the kernel's converter warps recover x = word - 0x1000 and l = x - h exactly.
+__device__ __forceinline__ float biased_word(double x) { return __uint_as_float(__float_as_uint((float)x) + 0x1000u); }
 
 // element k of the row starting at row_off (in elements)
 template <typename TO> struct Splitter;
@@ -35,8 +21,8 @@ template <> struct Splitter<double> {
     static __device__ __forceinline__ void put(double* hi, double*, size_t row_off, int k, double x) { hi[row_off + k] = x; }
 };
 template <> struct Splitter<float> {
-    static __device__ __forceinline__ void put(float* hi, float* pk, size_t row_off, int k, double x) {
-        put_split(hi, pk, row_off, k, x);
+    static __device__ __forceinline__ void put(float* hi, float*, size_t row_off, int k, double x) {
+        hi[row_off + k] = biased_word(x);
     }
 };
 
@@ -107,10 +93,10 @@ __global__ void pack_t2_kernel(const double* __restrict__ t2, size_t rows, int v
 }
 
 // ------------------------------------------------------------------------------------------------ mixed path
-// K-major FP32 operands of gemm_tf32.cuh, each as a pair (TF32 array, packed BF16 hi|lo array; put_split):
-//   XK  [r][b][c][d] = vvvo[d][b][c][r] = (db|cr)      (c: vp rows per b, d-pitch vk = v rounded up to 32)
+// K-major operands of gemm_tf32.cuh, 4 bytes per element (biased_word):
+//   XK  [r][b][c][d] = vvvo[d][b][c][r] = (db|cr)      (c: vp rows per b, d-pitch vk = v rounded up to 4)
 //   XKT [r][b][c][d] = XK[r][c][b][d]
-//   T2K [q][b][c][l] = t2[q][l][b][c]                  (l-pitch ok = o rounded up to 32)
+//   T2K [q][b][c][l] = t2[q][l][b][c]                  (l-pitch ok = o rounded up to 4)
 //   T2KT[r][b][c][l] = t2[l][r][b][c] = t2[r][l][c][b]
 //   T2A = pack_t2_kernel with pitch vk, OtA = pack_ot_kernel with pitch ok.
 // Pads are zeroed by the caller (cudaMemsetAsync) when any exists.
@@ -122,7 +108,7 @@ constexpr int PKX_PITCH = PKX_SPAN + 1;
 constexpr int PKX_SMEM = 32 * PKX_PITCH * 8;
 __global__ void __launch_bounds__(256)
 pack_xk_kernel(const double* __restrict__ vvvo, int v, int vp, int vk, int o, float* __restrict__ XK,
-               float* __restrict__ XKlo, float* __restrict__ XKT, float* __restrict__ XKTlo) {
+               float* __restrict__ XKT) {
     extern __shared__ double tile[];                 // [32][PKX_PITCH]
     const int d0 = blockIdx.y * 32;
     const size_t S = (size_t)v * v * o;
@@ -142,8 +128,9 @@ pack_xk_kernel(const double* __restrict__ vvvo, int v, int vp, int vk, int o, fl
         const size_t bc = sg / o;
         const int b = (int)(bc / v), c = (int)(bc % v);
         const double x = tile[dd * PKX_PITCH + s];
-        put_split(XK, XKlo, (size_t)r * plane + ((size_t)b * vp + c) * vk, d0 + dd, x);
-        put_split(XKT, XKTlo, (size_t)r * plane + ((size_t)c * vp + b) * vk, d0 + dd, x);
+        const float wd = biased_word(x);
+        XK[(size_t)r * plane + ((size_t)b * vp + c) * vk + d0 + dd] = wd;
+        XKT[(size_t)r * plane + ((size_t)c * vp + b) * vk + d0 + dd] = wd;
     }
 }
 
@@ -151,7 +138,7 @@ pack_xk_kernel(const double* __restrict__ vvvo, int v, int vp, int vk, int o, fl
 // blockIdx.z = chunk of 64 along l.
 __global__ void __launch_bounds__(256)
 pack_t2k_kernel(const double* __restrict__ t2, int v, int vp, int o, int ok, float* __restrict__ T2K,
-                float* __restrict__ T2Klo, float* __restrict__ T2KT, float* __restrict__ T2KTlo) {
+                float* __restrict__ T2KT) {
     __shared__ double tile[64][65];
     const int q = blockIdx.x / v, x = blockIdx.x % v;
     const int y0 = blockIdx.y * 64, l0 = blockIdx.z * 64;
@@ -164,8 +151,9 @@ pack_t2k_kernel(const double* __restrict__ t2, int v, int vp, int o, int ok, flo
     for (int e = threadIdx.x; e < nl * ny; e += 256) {
         const int l = e % nl, yy = e / nl;
         const double val = tile[l][yy];
-        put_split(T2K, T2Klo, (((size_t)q * v + x) * vp + (y0 + yy)) * ok, l0 + l, val);    // T2K [q][b=x][c=y][l]
-        put_split(T2KT, T2KTlo, (((size_t)q * v + (y0 + yy)) * vp + x) * ok, l0 + l, val);  // T2KT[q][b=y][c=x][l] = t2[q][l][x][y]
+        const float wd = biased_word(val);
+        T2K[(((size_t)q * v + x) * vp + (y0 + yy)) * ok + l0 + l] = wd;     // T2K [q][b=x][c=y][l]
+        T2KT[(((size_t)q * v + (y0 + yy)) * vp + x) * ok + l0 + l] = wd;    // T2KT[q][b=y][c=x][l] = t2[q][l][x][y]
     }
 }
 

@@ -131,8 +131,7 @@ int launch_gemm_f64(const GemmMaps& maps, const GemmJob* jobs, int njobs, const 
 
 struct Operands {   // device pointers of the repacked operands (workspace) for one precision
     void *x, *xt, *ot, *t2;
-    void *xlo, *xtlo, *otlo, *t2lo;
-    void *t2k, *t2kt, *t2klo, *t2ktlo;   // mixed path only
+    void *t2k, *t2kt;   // mixed path only
 };
 
 struct Maps {   // tensor maps of the contraction kernel of the plan's precision
@@ -156,24 +155,14 @@ int build_maps_f64(const Plan& P, const Operands& op, GemmMaps* maps) {
 int build_maps_tf32(const Plan& P, const Operands& op, Tf32Maps* maps) {
     const uint64_t o = P.o, v = P.v, vk = P.vk, ok = P.ok, NR = (uint64_t)P.v * P.vp;
     const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
-    const void* xk[2] = {op.x, op.xlo};
-    const void* xkt[2] = {op.xt, op.xtlo};
-    const void* t2k[2] = {op.t2k, op.t2klo};
-    const void* t2kt[2] = {op.t2kt, op.t2ktlo};
-    const void* t2a[2] = {op.t2, op.t2lo};
-    const void* ota[2] = {op.ot, op.otlo};
     int rc;
-    for (int h = 0; h < 2; ++h) {
-        // h = 0: TF32 arrays, K extent = v / o (TMA zero-fills the rest of the last chunk);  h = 1: packed BF16 hi|lo
-        // arrays, whole 32-float chunks (their pads are zeroed by prepare), so the K extent is the pitch
-        const uint64_t kv = h ? vk : v, ko = h ? ok : o;
-        if ((rc = make_map3(&maps->xk[h], dt, 4, xk[h], kv, NR, o, vk, NR * vk, TF_BK, TF_BM, 1))) return rc;
-        if ((rc = make_map3(&maps->xkt[h], dt, 4, xkt[h], kv, NR, o, vk, NR * vk, TF_BK, TF_BM, 1))) return rc;
-        if ((rc = make_map3(&maps->t2k[h], dt, 4, t2k[h], ko, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
-        if ((rc = make_map3(&maps->t2kt[h], dt, 4, t2kt[h], ko, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
-        if ((rc = make_map3(&maps->t2a[h], dt, 4, t2a[h], kv, v, o * o, vk, v * vk, TF_BK, P.tf_npad, 1))) return rc;
-        if ((rc = make_map3(&maps->ota[h], dt, 4, ota[h], ko, v, o * o, ok, v * ok, TF_BK, P.tf_npad, 1))) return rc;
-    }
+    // K extent = v / o: TMA zero-fills the rest of the last 32-wide chunk
+    if ((rc = make_map3(&maps->xk, dt, 4, op.x, v, NR, o, vk, NR * vk, TF_BK, TF_BM, 1))) return rc;
+    if ((rc = make_map3(&maps->xkt, dt, 4, op.xt, v, NR, o, vk, NR * vk, TF_BK, TF_BM, 1))) return rc;
+    if ((rc = make_map3(&maps->t2k, dt, 4, op.t2k, o, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
+    if ((rc = make_map3(&maps->t2kt, dt, 4, op.t2kt, o, NR, o, ok, NR * ok, TF_BK, TF_BM, 1))) return rc;
+    if ((rc = make_map3(&maps->t2a, dt, 4, op.t2, v, v, o * o, vk, v * vk, TF_BK, P.tf_npad, 1))) return rc;
+    if ((rc = make_map3(&maps->ota, dt, 4, op.ot, o, v, o * o, ok, v * ok, TF_BK, P.tf_npad, 1))) return rc;
     return TRIPLES_OK;
 }
 
@@ -229,14 +218,16 @@ int launch_gemm(const Plan& P, const Maps& maps, const GemmJob* jobs, int njobs,
 int run_prepare_mixed(const Plan& P, const double* t2, const double* vvvo, const double* ovoo, const Operands& op,
                       cudaStream_t st) {
     const int o = P.o, v = P.v;
-    if (P.vp != v || P.vk != v) {
-        for (void* ptr : {op.x, op.xlo, op.xt, op.xtlo}) CU_TRY(cudaMemsetAsync(ptr, 0, P.n_x * 4, st));
-        for (void* ptr : {op.t2, op.t2lo}) CU_TRY(cudaMemsetAsync(ptr, 0, P.n_t2 * 4, st));
+    if (P.vp != v || P.vk != v) {   // pads are zero words (the converter warps treat them as 0)
+        CU_TRY(cudaMemsetAsync(op.x, 0, P.n_x * 4, st));
+        CU_TRY(cudaMemsetAsync(op.xt, 0, P.n_x * 4, st));
+        CU_TRY(cudaMemsetAsync(op.t2, 0, P.n_t2 * 4, st));
     }
-    if (P.vp != v || P.ok != o)
-        for (void* ptr : {op.t2k, op.t2klo, op.t2kt, op.t2ktlo}) CU_TRY(cudaMemsetAsync(ptr, 0, P.n_t2k * 4, st));
-    if (P.ok != o)
-        for (void* ptr : {op.ot, op.otlo}) CU_TRY(cudaMemsetAsync(ptr, 0, P.n_ot * 4, st));
+    if (P.vp != v || P.ok != o) {
+        CU_TRY(cudaMemsetAsync(op.t2k, 0, P.n_t2k * 4, st));
+        CU_TRY(cudaMemsetAsync(op.t2kt, 0, P.n_t2k * 4, st));
+    }
+    if (P.ok != o) CU_TRY(cudaMemsetAsync(op.ot, 0, P.n_ot * 4, st));
     {
         static bool attr_set = false;
         if (!attr_set) {
@@ -245,22 +236,20 @@ int run_prepare_mixed(const Plan& P, const double* t2, const double* vvvo, const
         }
         const size_t S = (size_t)v * v * o;
         dim3 grid((unsigned)((S + PKX_SPAN - 1) / PKX_SPAN), (v + 31) / 32);
-        pack_xk_kernel<<<grid, 256, PKX_SMEM, st>>>(vvvo, v, P.vp, P.vk, o, (float*)op.x, (float*)op.xlo, (float*)op.xt,
-                                                    (float*)op.xtlo);
+        pack_xk_kernel<<<grid, 256, PKX_SMEM, st>>>(vvvo, v, P.vp, P.vk, o, (float*)op.x, (float*)op.xt);
         CU_TRY(cudaGetLastError());
         ++g_launches;
     }
     {
         dim3 grid(o * v, (v + 63) / 64, (o + 63) / 64);
-        pack_t2k_kernel<<<grid, 256, 0, st>>>(t2, v, P.vp, o, P.ok, (float*)op.t2k, (float*)op.t2klo, (float*)op.t2kt,
-                                              (float*)op.t2ktlo);
+        pack_t2k_kernel<<<grid, 256, 0, st>>>(t2, v, P.vp, o, P.ok, (float*)op.t2k, (float*)op.t2kt);
         CU_TRY(cudaGetLastError());
         ++g_launches;
     }
-    pack_ot_kernel<float><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.ok, (float*)op.ot, (float*)op.otlo);
+    pack_ot_kernel<float><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.ok, (float*)op.ot, nullptr);
     CU_TRY(cudaGetLastError());
     ++g_launches;
-    pack_t2_kernel<float><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vk, (float*)op.t2, (float*)op.t2lo);
+    pack_t2_kernel<float><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vk, (float*)op.t2, nullptr);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     return TRIPLES_OK;
@@ -284,7 +273,7 @@ int run_prepare(const Plan& P, const double* t2, const double* vvvo, const doubl
         const size_t smem = (size_t)RB * (o + 1) * 8;
         auto kern = pack_x_kernel<TO>;
         CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
-        kern<<<(unsigned)((R + RB - 1) / RB), 256, smem, st>>>(vvvo, v, P.vp, o, RB, (TO*)op.x, (TO*)op.xlo);
+        kern<<<(unsigned)((R + RB - 1) / RB), 256, smem, st>>>(vvvo, v, P.vp, o, RB, (TO*)op.x, nullptr);
         CU_TRY(cudaGetLastError());
         ++g_launches;
     }
@@ -298,10 +287,10 @@ int run_prepare(const Plan& P, const double* t2, const double* vvvo, const doubl
         }
         CU_TRY(cudaGetLastError());
     }
-    pack_ot_kernel<TO><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.op, (TO*)op.ot, (TO*)op.otlo);
+    pack_ot_kernel<TO><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.op, (TO*)op.ot, nullptr);
     CU_TRY(cudaGetLastError());
     ++g_launches;
-    pack_t2_kernel<TO><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vp, (TO*)op.t2, (TO*)op.t2lo);
+    pack_t2_kernel<TO><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vp, (TO*)op.t2, nullptr);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     return TRIPLES_OK;
@@ -310,10 +299,7 @@ int run_prepare(const Plan& P, const double* t2, const double* vvvo, const doubl
 Operands carve_operands(const Plan& P, uint8_t* ws) {
     Operands op{};
     op.x = ws + P.off_x; op.xt = ws + P.off_xt; op.ot = ws + P.off_ot; op.t2 = ws + P.off_t2;
-    if (P.prec == TRIPLES_MIXED) {
-        op.xlo = ws + P.off_xlo; op.xtlo = ws + P.off_xtlo; op.otlo = ws + P.off_otlo; op.t2lo = ws + P.off_t2lo;
-        op.t2k = ws + P.off_t2k; op.t2kt = ws + P.off_t2kt; op.t2klo = ws + P.off_t2klo; op.t2ktlo = ws + P.off_t2ktlo;
-    }
+    if (P.prec == TRIPLES_MIXED) { op.t2k = ws + P.off_t2k; op.t2kt = ws + P.off_t2kt; }
     return op;
 }
 

@@ -164,6 +164,9 @@ SAMPLES = {"small": 32, "medium": 24, "large": 7, "largest": 6}   # incl. 6 forc
 @pytest.mark.parametrize("name", ["small", "medium", "large", "largest"])
 def test_config_sampled_triplets(name, prec):
     o, v, naux = synth.CONFIGS[name]
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()      # blocks cached by earlier tests would count as "not free"
     free, _ = torch.cuda.mem_get_info()
     need = tb.triples_workspace_bytes(o, v, prec) + 8 * v ** 3 * o * 1.2
     if free < need:
