@@ -285,6 +285,21 @@ def main():
         "avg_launch_ms": prof["reduction_ms"] / max(prof["reduction_launches"], 1),
     }
 
+    # DRAM traffic per launch of the captured batch (ncu --set full summary committed under profiles/; medium only)
+    tpath = os.path.join(ROOT, "profiles", "r01_ncu_traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            tr = json.load(f).get(args.config, {})
+        g = tr.get(roofline["kernel"])
+        r = tr.get("reduce_kernel<double>" if prec == tb.FP64 else "reduce_kernel<float>")
+        if g:
+            roofline["traffic"] = g["dram_bytes"]
+            roofline["traffic_note"] = (f"ncu dram bytes of one captured launch ({g.get('jobs_in_launch')} jobs, "
+                                        "profiles/r01_ncu_full_medium.md); launches differ in size")
+        if r:
+            roofline_reduction["traffic"] = r["dram_bytes"]
+            roofline_reduction["traffic_note"] = "ncu dram bytes of one captured launch (profiles/r01_ncu_full_medium.md)"
+
     # ---- end-to-end: host (pinned) inputs through triples_energy_host, copies inside the timed region
     e2e = None
     if not args.no_e2e:

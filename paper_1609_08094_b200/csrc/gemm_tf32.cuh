@@ -18,29 +18,33 @@
 // Operands are K-major arrays (prepare.cuh): XK[r][b][c][d] = (db|cr), XKT[r][b][c][d] = XK[r][c][b][d],
 // T2A[p][q][a][d] = t2, OtA[r][p][a][l] = -(pa|lr), T2K[q][b][c][l] = t2[q,l,b,c], T2KT[r][b][c][l] = t2[l,r,b,c];
 // the c index has vp rows per b (row v is zero when v is odd) so that U keeps the pitch the reduction expects.
-// Each exists twice with the same geometry (rows of 32-float = 128-byte K chunks): the TF32 values h, and a packed
-// array whose chunk holds 32 BF16 of h (bytes 0..63) followed by 32 BF16 of l (bytes 64..127).
+// An element is ONE 4-byte word: the FP32 bit pattern of x plus 0x1000 (prepare.cuh biased_word).  The TF32 MMA
+// ignores the low 13 bits of its operands, so it reads the word as h = RN_tf32(x) straight from the TMA-written tile;
+// converter warps recover x and l = x - h exactly and write, per 32-wide K chunk, a packed tile whose 128-byte rows
+// hold 32 BF16 of h (bytes 0..63) and 32 BF16 of l (bytes 64..127) for the cross-term MMAs.  Splitting inside the
+// SM halves the operand bytes in HBM and through L2 (with separate hi/lo arrays the loop was bound by the ~42
+// B/clk/SM L2 -> SM cap, not by the tensor pipe).
 //
 // The kernel is persistent and runs as CTA PAIRS (thread-block clusters of 2 = the two SMs of a TPC, cta_group::2):
 // a pair walks work items (job, two consecutive m-tiles of 128 (b,c) rows, n-tile of BN a-columns) as ONE
 // 256 x BN MMA tile.  Each CTA stages only its own 128 M-side rows and HALF of the N-side rows (the tensor cores
-// read the other half from the peer's shared memory), which cuts the bytes an SM pulls in per MMA by a third: at
-// 8 bytes per operand element the loop is bound by L2 -> SM throughput (~42 B/clk/SM chip-wide cap), not by the
-// tensor pipe.  Jobs of a launch are grouped by (q,r) so that the big XK_r / XKT_q slices come from HBM once per
-// group (tf32_item below).
-//   warp 0    : TMA producer   (K chunks of 32 floats = one 128-byte swizzled row per operand row; TF32 and packed
-//                               tiles; both CTAs load, the transaction bytes all count on the leader's barrier)
+// read the other half from the peer's shared memory).  Jobs of a launch are grouped by (q,r) so that the big
+// XK_r / XKT_q slices come from HBM once per group (tf32_item below).
+//   warp 0    : TMA producer   (K chunks of 32 words = one 128-byte swizzled row per operand row, ring of 4 raw tiles)
 //   warp 1    : MMA issuer     (one lane of the LEADER CTA; per K chunk 2+2 BF16 cross-term MMAs (K = 16), then 4
 //                               TF32 MMAs (K = 8); tcgen05.commit multicasts to both CTAs' barriers)
-//   warp 2    : TMEM allocator (512 columns = two 128 x 256 FP32 buffers in each CTA)
-//   warps 4-11: accumulators   (tcgen05.ld of every finished chain, FP32 round-to-nearest adds in registers,
+//   warps 2-7 : converters     (raw tile -> packed BF16 tile, ring of 2; warp 2 also allocates TMEM: 512 columns =
+//                               two 128 x 256 FP32 buffers in each CTA)
+//   warps 8-15: accumulators   (tcgen05.ld of every finished chain, FP32 round-to-nearest adds in registers,
 //                               one 256-bit store per (b,c) row and a-tile of U at the end of the item)
 //
 // Why the running sum lives in registers and not in TMEM: the tensor core adds each MMA's result to its accumulator
 // with truncation, so one long accumulation chain is biased towards zero by ~(number of MMAs) * 2^-25 (measured:
 // -3.4e-6 relative on W at v = 240, i.e. 7e-6 on E(T), growing with v).  A TMEM buffer therefore only ever holds a
-// short chain (TF_CHAIN K chunks, started with accumulate = 0, the small cross terms first); finished chains
-// are added with FADD.RN by the accumulator warps while the tensor core fills the other buffer.
+// short chain (TF_CHAIN = 2 K chunks = 16 MMAs, started with accumulate = 0, cross terms before the main term of
+// each chunk); finished chains are added with FADD.RN by the accumulator warps while the tensor core fills the
+// other buffer.  Measured bias on E(T): 1.8e-7 with one chunk per chain, 4.7e-7 with two (8 % faster: the kernel
+// runs at the 1 kW power cap and every chain costs a 128 x BN TMEM read-out); tolerance 1e-5.
 #pragma once
 #include "gemm_f64.cuh"   // GemmJob
 #include "ptx.cuh"
@@ -61,7 +65,7 @@ constexpr int TF_BM = 128;            // (b,c) rows per CTA tile = TMEM lanes
 constexpr int TF_BK = 32;             // floats per K chunk (128-byte rows)
 constexpr int TF_THREADS = 512;         // 8 service warps (TMA, MMA, TMEM, 4 converters) + 8 accumulator warps
 constexpr int TF_CONV_WARPS = 6;        // warps 2..7
-constexpr int TF_CHAIN = 1;             // K chunks per TMEM accumulation chain
+constexpr int TF_CHAIN = 2;             // K chunks per TMEM accumulation chain
 constexpr int TF_TMEM_COLS = 512;
 constexpr int TF_SMEM_LIMIT = 227 * 1024;
 constexpr int TF_MAX_JOBS = 192;        // jobs per launch (3 per triplet, plan.h: at most 4^3 triplets per batch); the
