@@ -138,6 +138,21 @@ int triples_w_block(int nocc, int nvirt,
 int triples_last_profile(double* out10);
 void triples_set_profiling(int on);
 
+/*
+ * Host-side planner (S1; Eq. (5.0.7b)): how triples_energy cuts the restricted loop into
+ * launches. Pure host arithmetic, no GPU needed. A batch is the set of restricted triplets of one block
+ * I x J x K of occupied-index windows; inside a batch the contraction jobs G(p,q,r) are sorted by (q,r)
+ * and the jobs sharing (q,r) -- the same (vv|vo) slices -- form a group that the kernels walk together.
+ *   batch_of_triplet : host, T ints or NULL: batch of triplet n of triples_triplet_list (-1 for i=j=k,
+ *                      which contributes exactly zero and is skipped)
+ *   jobs_out         : host, 3*T*6 ints or NULL: per job, in launch order,
+ *                      {batch, p, q, r, first job of its group (relative to the batch), group size}
+ *   njobs_out        : host or NULL: number of jobs (<= 3*T; a triplet with i=j or j=k has two)
+ * Returns the number of batches, or -1 on invalid sizes / precision (message in triples_last_error).
+ */
+long long triples_plan_batches(int nocc, int nvirt, int precision, int* batch_of_triplet, int* jobs_out,
+                               long long* njobs_out);
+
 /* Number of CUDA kernels the calling thread's last compute call (triples_energy / _host / _subset / _w_block)
  * launched (repack + contraction + reduction + finalize + total). */
 long long triples_last_launch_count(void);

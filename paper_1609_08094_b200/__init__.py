@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     triples_energy_subset,
     triples_last_launch_count,
     triples_last_profile,
+    triples_plan_batches,
     triples_set_profiling,
     triples_triplet_count,
     triples_triplet_list,

@@ -46,6 +46,9 @@ def lib() -> ctypes.CDLL:
         L.triples_triplet_count.restype = ctypes.c_longlong
         L.triples_triplet_list.argtypes = [ctypes.c_int, ip]
         L.triples_triplet_list.restype = ctypes.c_int
+        L.triples_plan_batches.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ip, ip,
+                                           ctypes.POINTER(ctypes.c_longlong)]
+        L.triples_plan_batches.restype = ctypes.c_longlong
         for name in ("triples_workspace_bytes", "triples_workspace_bytes_host"):
             f = getattr(L, name)
             f.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int]
@@ -134,6 +137,20 @@ def triples_last_profile() -> dict:
     keys = ("prepare_ms", "contraction_ms", "contraction_launches", "reduction_ms", "reduction_launches",
             "other_ms", "other_launches", "contraction_flops", "reduction_bytes", "triplets")
     return dict(zip(keys, [float(x) for x in out]))
+
+
+def triples_plan_batches(nocc: int, nvirt: int, precision: int):
+    """(number of batches, batch_of_triplet[T], jobs[njobs, 6] = {batch, p, q, r, group_start, group_size})."""
+    T = triples_triplet_count(nocc)
+    bot = np.empty(T, dtype=np.int32)
+    jobs = np.empty((3 * T, 6), dtype=np.int32)
+    nj = ctypes.c_longlong(0)
+    ip = ctypes.POINTER(ctypes.c_int)
+    nb = lib().triples_plan_batches(nocc, nvirt, precision, bot.ctypes.data_as(ip), jobs.ctypes.data_as(ip),
+                                    ctypes.byref(nj))
+    if nb < 0:
+        raise TriplesError(1, lib().triples_last_error().decode())
+    return int(nb), bot, jobs[: nj.value].copy()
 
 
 def triples_last_launch_count() -> int:

@@ -2,6 +2,7 @@
 // Pure host arithmetic (no CUDA calls) so that the CPU test-suite can exercise it through the C ABI.
 #pragma once
 #include <cstddef>
+#include <algorithm>
 #include <cstdint>
 #include <cstdlib>
 #include <vector>
@@ -175,6 +176,72 @@ inline bool make_plan(int o, int v, int prec, Plan& P) {
     for (int n = 0; n < 7; ++n) { P.in_bytes[n] = in_elems[n] * 8; P.off_in[n] = take(P.in_bytes[n]); }
     P.total_host = off;
     return true;
+}
+
+// ------------------------------------------------------------------------------------------------ batches (S1)
+// One contraction job G(p,q,r) of a batch.  u / u2: which of the triplet slot's three U
+// buffers receive it (u2 = -1 unless a coinciding pair i=j or j=k makes one G serve two of them).
+struct JobDesc { int p, q, r, slot, u, u2, gstart, gsize; };
+
+struct BatchPlan {
+    std::vector<Triplet> work;     // triplets in execution order (i=j=k dropped: they contribute exactly zero)
+    std::vector<size_t> bstart;    // batch b = work[bstart[b] .. bstart[b+1]); slot of a triplet = offset in its batch
+    std::vector<JobDesc> jobs;     // jobs of all batches; inside a batch sorted by (q,r,p)
+    std::vector<int> jstart;       // batch b = jobs[jstart[b] .. jstart[b+1]); gstart is relative to jstart[b]
+    double distinct_u = 0.0;       // U buffers the reductions read (2 per triplet with a coinciding pair, else 3)
+};
+
+// Batches = the triplets of one block I x J x K of occupied-index windows of width P.win (at most P.nb each).
+// Inside a batch the jobs with the same (q,r) -- the same X_r / XT_q operand slices -- form one group.
+inline void build_batches(const Plan& P, const std::vector<Triplet>& trip, BatchPlan& B) {
+    B = BatchPlan();
+    for (const Triplet& t : trip)
+        if (!(t.i == t.j && t.j == t.k)) B.work.push_back(t);
+    const int win = P.win, nwin = (P.o + win - 1) / win;
+    auto key = [&](const Triplet& t) { return ((long long)(t.i / win) * nwin + t.j / win) * nwin + t.k / win; };
+    // stable: inside a block the enumeration order of the caller's list is kept
+    std::vector<Triplet> sorted(B.work);
+    std::vector<long long> keys(sorted.size());
+    for (size_t n = 0; n < sorted.size(); ++n) keys[n] = key(sorted[n]);
+    std::vector<size_t> order(sorted.size());
+    for (size_t n = 0; n < order.size(); ++n) order[n] = n;
+    std::stable_sort(order.begin(), order.end(), [&](size_t x, size_t y) { return keys[x] < keys[y]; });
+    for (size_t n = 0; n < order.size(); ++n) B.work[n] = sorted[order[n]];
+    const size_t nwork = B.work.size();
+    for (size_t n = 0; n < nwork; ++n)
+        if (n == 0 || key(B.work[n]) != key(B.work[n - 1]) || n - B.bstart.back() == (size_t)P.nb) B.bstart.push_back(n);
+    B.bstart.push_back(nwork);
+    const size_t nbatch = B.bstart.size() - 1;
+    for (size_t b = 0; b < nbatch; ++b) {
+        const size_t j0 = B.jobs.size();
+        B.jstart.push_back((int)j0);
+        for (size_t n = B.bstart[b]; n < B.bstart[b + 1]; ++n) {
+            const Triplet& t = B.work[n];
+            const int slot = (int)(n - B.bstart[b]);
+            if (t.i == t.j) {            // G(j,i,k) = G(i,j,k): one job, two destinations
+                B.jobs.push_back({t.i, t.j, t.k, slot, 0, 1, 0, 1});
+                B.jobs.push_back({t.k, t.i, t.j, slot, 2, -1, 0, 1});
+            } else if (t.j == t.k) {     // G(k,i,j) = G(j,i,k)
+                B.jobs.push_back({t.i, t.j, t.k, slot, 0, -1, 0, 1});
+                B.jobs.push_back({t.j, t.i, t.k, slot, 1, 2, 0, 1});
+            } else {
+                B.jobs.push_back({t.i, t.j, t.k, slot, 0, -1, 0, 1});   // U1 = G(i,j,k)[a][b][c]
+                B.jobs.push_back({t.j, t.i, t.k, slot, 1, -1, 0, 1});   // U2 = G(j,i,k)[b][a][c]
+                B.jobs.push_back({t.k, t.i, t.j, slot, 2, -1, 0, 1});   // U3 = G(k,i,j)[c][a][b]
+            }
+            B.distinct_u += 1.0 + (t.i != t.j) + (t.j != t.k);
+        }
+        std::sort(B.jobs.begin() + j0, B.jobs.end(), [](const JobDesc& x, const JobDesc& y) {
+            return x.q != y.q ? x.q < y.q : (x.r != y.r ? x.r < y.r : (x.p != y.p ? x.p < y.p : x.slot < y.slot));
+        });
+        for (size_t g = j0; g < B.jobs.size();) {
+            size_t e = g;
+            while (e < B.jobs.size() && B.jobs[e].q == B.jobs[g].q && B.jobs[e].r == B.jobs[g].r) ++e;
+            for (size_t x = g; x < e; ++x) { B.jobs[x].gstart = (int)(g - j0); B.jobs[x].gsize = (int)(e - g); }
+            g = e;
+        }
+    }
+    B.jstart.push_back((int)B.jobs.size());
 }
 
 }  // namespace tb

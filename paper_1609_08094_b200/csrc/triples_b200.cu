@@ -329,64 +329,33 @@ int run_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, c
     Maps maps;
     if (int rc = build_maps(P, op, &maps)) return rc;
 
-    // ---- job tables for every batch, uploaded once
+    // ---- batches and job tables (plan.h), uploaded once
     std::vector<Orbit> orbits;
     enumerate_orbits(v, orbits);
-    std::vector<Triplet> work;   // i=j=k contributes exactly zero (weight 0, Q5): skipped
-    for (const Triplet& t : trip)
-        if (!(t.i == t.j && t.j == t.k)) work.push_back(t);
-    const size_t nwork = work.size();
-    // batches (S1): the triplets of one block of occupied-index windows (plan.h), at most P.nb of them
-    const int win = P.win, nwin = (o + win - 1) / win;
-    auto block_key = [&](const Triplet& t) { return ((long long)(t.i / win) * nwin + t.j / win) * nwin + t.k / win; };
-    std::stable_sort(work.begin(), work.end(),
-                     [&](const Triplet& x, const Triplet& y) { return block_key(x) < block_key(y); });
-    std::vector<size_t> bstart;   // first triplet of each batch
-    for (size_t n = 0; n < nwork; ++n)
-        if (n == 0 || block_key(work[n]) != block_key(work[n - 1]) || n - bstart.back() == (size_t)P.nb) bstart.push_back(n);
-    bstart.push_back(nwork);
-    const size_t nbatch = bstart.size() - 1;
-    std::vector<GemmJob> gj;
+    BatchPlan B;
+    build_batches(P, trip, B);
+    const std::vector<Triplet>& work = B.work;
+    const std::vector<size_t>& bstart = B.bstart;
+    const std::vector<int>& gj_begin = B.jstart;
+    const size_t nwork = work.size(), nbatch = bstart.size() - 1;
+    const double distinct_u = B.distinct_u;
+    TS* ubase = reinterpret_cast<TS*>(ws + P.off_u);
+    std::vector<GemmJob> gj(B.jobs.size());
+    for (size_t n = 0; n < gj.size(); ++n) {
+        const JobDesc& d = B.jobs[n];
+        TS* ub = ubase + (size_t)3 * d.slot * P.n_u;      // interleaved blocks of U1,U2,U3 of the slot (ulayout.cuh)
+        gj[n] = {d.p, d.q, d.r, d.gstart, ub + (size_t)d.u * UBLK, d.u2 < 0 ? nullptr : ub + (size_t)d.u2 * UBLK,
+                 d.gsize, {0, 0, 0}};
+    }
     std::vector<RedJob> rj(nwork);
     std::vector<FinJob> fj(nwork);
-    std::vector<int> gj_begin;   // first gemm job of each batch
-    TS* ubase = reinterpret_cast<TS*>(ws + P.off_u);
-    double distinct_u = 0.0;
-    for (size_t b = 0; b < nbatch; ++b) {
-        const size_t j0 = gj.size();
-        gj_begin.push_back((int)j0);
+    for (size_t b = 0; b < nbatch; ++b)
         for (size_t n = bstart[b]; n < bstart[b + 1]; ++n) {
             const Triplet& t = work[n];
             const int slot = (int)(n - bstart[b]);
-            TS* ub = ubase + (size_t)3 * slot * P.n_u;                 // interleaved blocks of U1,U2,U3 (ulayout.cuh)
-            TS *u1 = ub, *u2 = ub + UBLK, *u3 = ub + 2 * UBLK;
-            if (t.i == t.j) {            // G(j,i,k) = G(i,j,k): one job, two destinations
-                gj.push_back({t.i, t.j, t.k, 0, u1, u2, 1, {0, 0, 0}});
-                gj.push_back({t.k, t.i, t.j, 0, u3, nullptr, 1, {0, 0, 0}});
-            } else if (t.j == t.k) {     // G(k,i,j) = G(j,i,k)
-                gj.push_back({t.i, t.j, t.k, 0, u1, nullptr, 1, {0, 0, 0}});
-                gj.push_back({t.j, t.i, t.k, 0, u2, u3, 1, {0, 0, 0}});
-            } else {
-                gj.push_back({t.i, t.j, t.k, 0, u1, nullptr, 1, {0, 0, 0}});               // G(i,j,k)[a][b][c]
-                gj.push_back({t.j, t.i, t.k, 0, u2, nullptr, 1, {0, 0, 0}});               // G(j,i,k)[b][a][c]
-                gj.push_back({t.k, t.i, t.j, 0, u3, nullptr, 1, {0, 0, 0}});               // G(k,i,j)[c][a][b]
-            }
-            distinct_u += 1.0 + (t.i != t.j) + (t.j != t.k);
-            rj[n] = {t.i, t.j, t.k, slot, ub, nullptr};
+            rj[n] = {t.i, t.j, t.k, slot, ubase + (size_t)3 * slot * P.n_u, nullptr};
             fj[n] = {slot, (int)t.index, triplet_weight(t.i, t.j, t.k)};
         }
-        // jobs with the same (q,r) read the same X_r / XT_q slices: make them neighbours and tell the kernel
-        std::sort(gj.begin() + j0, gj.end(), [](const GemmJob& x, const GemmJob& y) {
-            return x.q != y.q ? x.q < y.q : (x.r != y.r ? x.r < y.r : x.p < y.p);
-        });
-        for (size_t g = j0; g < gj.size();) {
-            size_t e = g;
-            while (e < gj.size() && gj[e].q == gj[g].q && gj[e].r == gj[g].r) ++e;
-            for (size_t x = g; x < e; ++x) { gj[x].gstart = (int)(g - j0); gj[x].gsize = (int)(e - g); }
-            g = e;
-        }
-    }
-    gj_begin.push_back((int)gj.size());
     GemmJob* d_gj = reinterpret_cast<GemmJob*>(ws + P.off_gjobs);
     RedJob* d_rj = reinterpret_cast<RedJob*>(ws + P.off_rjobs);
     double* d_side = reinterpret_cast<double*>(ws + P.off_side);
@@ -513,6 +482,34 @@ int triples_triplet_list(int nocc, int* ijk_out) {
     enumerate_triplets(nocc, t);
     for (size_t n = 0; n < t.size(); ++n) { ijk_out[3 * n] = t[n].i; ijk_out[3 * n + 1] = t[n].j; ijk_out[3 * n + 2] = t[n].k; }
     return TRIPLES_OK;
+}
+
+long long triples_plan_batches(int nocc, int nvirt, int precision, int* batch_of_triplet, int* jobs_out,
+                               long long* njobs_out) {
+    Plan P;
+    if (!make_plan(nocc, nvirt, precision, P)) {
+        fail(TRIPLES_EINVAL, "invalid sizes/precision: nocc=%d nvirt=%d precision=%d", nocc, nvirt, precision);
+        return -1;
+    }
+    std::vector<Triplet> trip;
+    enumerate_triplets(nocc, trip);
+    BatchPlan B;
+    build_batches(P, trip, B);
+    const size_t nbatch = B.bstart.size() - 1;
+    if (batch_of_triplet) {
+        for (long long n = 0; n < P.T; ++n) batch_of_triplet[n] = -1;
+        for (size_t b = 0; b < nbatch; ++b)
+            for (size_t n = B.bstart[b]; n < B.bstart[b + 1]; ++n) batch_of_triplet[B.work[n].index] = (int)b;
+    }
+    if (jobs_out)
+        for (size_t b = 0; b < nbatch; ++b)
+            for (int g = B.jstart[b]; g < B.jstart[b + 1]; ++g) {
+                const JobDesc& d = B.jobs[g];
+                int* o6 = jobs_out + 6 * (size_t)g;
+                o6[0] = (int)b; o6[1] = d.p; o6[2] = d.q; o6[3] = d.r; o6[4] = d.gstart; o6[5] = d.gsize;
+            }
+    if (njobs_out) *njobs_out = (long long)B.jobs.size();
+    return (long long)nbatch;
 }
 
 size_t triples_workspace_bytes(int nocc, int nvirt, int precision) {

@@ -125,3 +125,73 @@ def test_product_does_not_import_the_oracle():
             text = open(path).read()
             assert not re.search(r"^\s*(import|from)\s+paper_1609_08094_b200", text, flags=re.M), path
             assert "libtriples_b200" not in text and "triples_b200.h" not in text, path
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# host planner (S1): batches = blocks of occupied-index windows, contraction jobs grouped by (q,r)
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("o,v,prec", [(1, 6, 0), (2, 3, 0), (8, 40, 0), (8, 40, 1), (16, 120, 1), (24, 240, 0),
+                                      (24, 240, 1), (13, 50, 1), (40, 480, 1), (40, 480, 0), (32, 400, 0)])
+def test_batches_cover_every_triplet_once_and_jobs_are_grouped(o, v, prec):
+    nb, bot, jobs = tb.triples_plan_batches(o, v, prec)
+    trips = tb.triples_triplet_list(o)
+    T = len(trips)
+    diag = np.array([i == j == k for i, j, k in trips])
+    # i=j=k cycles contribute exactly zero (Q5) and are in no batch; every other cycle is in exactly one
+    assert np.all(bot[diag] == -1) and np.all(bot[~diag] >= 0)
+    if T == int(diag.sum()):
+        assert nb == 0 and len(jobs) == 0
+        return
+    assert set(bot[~diag].tolist()) == set(range(nb))
+    # a batch is one block of index windows of one width, at most 64 triplets
+    sizes = np.bincount(bot[~diag], minlength=nb)
+    assert sizes.max() <= 64
+    for w in (1, 2, 3, 4):
+        key = (trips[:, 0] // w) * 10000 + (trips[:, 1] // w) * 100 + trips[:, 2] // w
+        if all(len(set(key[(bot == b)].tolist())) == 1 for b in range(nb)) and \
+                len(set(zip(key[~diag].tolist(), bot[~diag].tolist()))) == nb:
+            break
+    else:
+        raise AssertionError("batches are not the blocks of any window width 1..4")
+    # jobs: every triplet gets G(i,j,k), G(j,i,k), G(k,i,j), coinciding ones once
+    want = {}
+    for n, (i, j, k) in enumerate(trips.tolist()):
+        if i == j == k:
+            continue
+        for g in {(i, j, k), (j, i, k), (k, i, j)}:
+            want[(int(bot[n]),) + g] = want.get((int(bot[n]),) + g, 0) + 1
+    got = {}
+    for b, p, q, r, gs, gn in jobs.tolist():
+        got[(b, p, q, r)] = got.get((b, p, q, r), 0) + 1
+    assert got == want
+    # launch order: batch by batch; inside a batch sorted by (q,r); group fields describe the runs of equal (q,r)
+    assert np.all(np.diff(jobs[:, 0]) >= 0)
+    for b in range(nb):
+        jb = jobs[jobs[:, 0] == b]
+        qr = [tuple(x) for x in jb[:, 2:4].tolist()]
+        assert qr == sorted(qr)
+        n = 0
+        while n < len(jb):
+            gs, gn = int(jb[n, 4]), int(jb[n, 5])
+            assert gs == n and gn >= 1
+            assert all(tuple(x) == qr[n] for x in jb[n:n + gn, 2:4].tolist())
+            assert np.all(jb[n:n + gn, 4] == gs) and np.all(jb[n:n + gn, 5] == gn)
+            assert n + gn == len(jb) or qr[n + gn] != qr[n]
+            n += gn
+
+
+def test_window_batches_share_operand_slices():
+    """medium config: blocks of width-4 windows, so a (q,r) group has up to 4 jobs (the (vv|vo) slices X_r, XT_q
+    are fetched once per group instead of once per job)."""
+    nb, bot, jobs = tb.triples_plan_batches(24, 240, 1)
+    assert nb == 56                                   # 6 windows: 6*7*8/6 blocks
+    gsz = jobs[:, 5]
+    assert gsz.max() == 4 and gsz.mean() > 3.0
+
+
+def test_plan_batches_rejects_bad_sizes(lib):
+    import ctypes
+    assert lib.triples_plan_batches(0, 5, 0, None, None, None) == -1
+    assert lib.triples_plan_batches(3, 5, 7, None, None, None) == -1
+    assert b"invalid" in lib.triples_last_error()
+    assert lib.triples_plan_batches(3, 5, 0, None, None, None) > 0
