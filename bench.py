@@ -179,6 +179,8 @@ def main():
     ap.add_argument("--cpu-triplets", type=int, default=4, help="triplets of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-mixed-leg", action="store_true",
+                    help="FP64 runs only: skip the extra mixed-precision measurement reported under 'mixed_path'")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -217,7 +219,11 @@ def main():
         if need_host:
             host = {k: dev[k].cpu().numpy() for k in NAMES}
     dargs = [dev[k] for k in NAMES]
-    ws = torch.empty(tb.triples_workspace_bytes_host(o, v, prec), dtype=torch.uint8, device="cuda")
+    mixed_leg = prec == tb.FP64 and world == 1 and not args.no_mixed_leg and args.config in ("tiny", "small", "medium")
+    ws_bytes = tb.triples_workspace_bytes_host(o, v, prec)
+    if mixed_leg:
+        ws_bytes = max(ws_bytes, tb.triples_workspace_bytes(o, v, tb.MIXED))
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -319,6 +325,40 @@ def main():
                "d2h_bytes_per_step": 24, "s_per_ET": sec_e_max / args.steps,
                "api": "triples_energy_host (C ABI, host buffers pinned)"}
 
+    # ---- the paper's other precision beside the headline one (its single/double study): same workload
+    mixed = None
+    if mixed_leg:
+        tb.triples_energy(o, v, *dargs, tb.MIXED, ws, stream=stream)            # warm-up
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        m0.record(stream)
+        for _ in range(args.steps):
+            Em = tb.triples_energy(o, v, *dargs, tb.MIXED, ws, stream=stream)
+        m1.record(stream)
+        torch.cuda.synchronize()
+        msec = m0.elapsed_time(m1) / 1e3 / args.steps
+        tb.triples_set_profiling(True)
+        tb.triples_energy(o, v, *dargs, tb.MIXED, ws, stream=stream)
+        mp = tb.triples_last_profile()
+        tb.triples_set_profiling(False)
+        mg = mp["contraction_flops"] / (mp["contraction_ms"] * 1e-3) / 1e12
+        mr = mp["reduction_bytes"] / (mp["reduction_ms"] * 1e-3) / 1e9
+        tf32_peak = peaks["bf16_tflops_sustained"] * 0.5
+        mixed = {"value": formula_flops(o, v) / msec / 1e12, "unit": "TFLOP/s", "s_per_ET": msec,
+                 "dtype": "tf32+bf16 split (f32 accumulate), f64 reduction",
+                 "E_T": Em[0], "E4": Em[1], "E5": Em[2],
+                 "rel_dev_from_fp64": {"E_T": abs(Em[0] - E[0]) / abs(E[0]), "E4": abs(Em[1] - E[1]) / abs(E[1]),
+                                       "E5_abs_dev_over_abs_E4": abs(Em[2] - E[2]) / abs(E[1]),
+                                       "note": "tolerance 1e-5 on E(T); E5 is 1e-7..1e-4 of E4 with the generator's "
+                                               "t1 ~ N(0,1e-3^2) and a sum of both signs, so its deviation is "
+                                               "given on the scale of E4 (tests pin E5 with t1 ~ N(0,1))"},
+                 "contraction": {"kernel": "gemm_tf32_kernel", "achieved": mg, "peak": tf32_peak, "unit": "TFLOP/s",
+                                 "frac": mg / tf32_peak, "frac_tensor_pipe": 2.0 * mg / tf32_peak,
+                                 "peak_note": "0.5 x measured sustained bf16; frac = algorithmic flops, "
+                                              "frac_tensor_pipe = TF32-rate-equivalent tensor work (DESIGN.md 7.2)"},
+                 "reduction": {"kernel": "reduce_kernel<float>", "achieved": mr, "peak": peaks["hbm_gbs"],
+                               "unit": "GB/s", "frac": mr / peaks["hbm_gbs"]}}
+
     # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample (rank 0, N=1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -348,6 +388,8 @@ def main():
             "phase_ms": {k: prof[k] for k in ("prepare_ms", "contraction_ms", "reduction_ms", "other_ms")},
             "e2e": e2e, "cpu_baseline": cpu,
         }
+        if mixed is not None:
+            line["mixed_path"] = mixed
         print(json.dumps(line), flush=True)
     if world > 1:
         import torch.distributed as dist

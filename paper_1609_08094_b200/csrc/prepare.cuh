@@ -15,21 +15,15 @@ namespace tb {
 // cvt.rna.tf32.f32 gives); the kernel's converter warps recover x = word - 0x1000 and l = x - h exactly.
 __device__ __forceinline__ float biased_word(double x) { return __uint_as_float(__float_as_uint((float)x) + 0x1000u); }
 
-// element k of the row starting at row_off (in elements)
-template <typename TO> struct Splitter;
-template <> struct Splitter<double> {
-    static __device__ __forceinline__ void put(double* hi, double*, size_t row_off, int k, double x) { hi[row_off + k] = x; }
-};
-template <> struct Splitter<float> {
-    static __device__ __forceinline__ void put(float* hi, float*, size_t row_off, int k, double x) {
-        hi[row_off + k] = biased_word(x);
-    }
-};
+// operand element of the contraction path: the double itself (FP64), or the mixed path's biased FP32 word
+template <typename TO> __device__ __forceinline__ TO operand_word(double x);
+template <> __device__ __forceinline__ double operand_word<double>(double x) { return x; }
+template <> __device__ __forceinline__ float operand_word<float>(double x) { return biased_word(x); }
 
 // vvvo viewed as [R = v^3][o]: each CTA moves RB consecutive rows (one contiguous span) through smem.
 template <typename TO>
 __global__ void __launch_bounds__(256)
-pack_x_kernel(const double* __restrict__ vvvo, int v, int vp, int o, int RB, TO* __restrict__ X, TO* __restrict__ Xlo) {
+pack_x_kernel(const double* __restrict__ vvvo, int v, int vp, int o, int RB, TO* __restrict__ X) {
     extern __shared__ double tile[];   // [RB][o+1]
     const size_t R = (size_t)v * v * v;
     const size_t R0 = (size_t)blockIdx.x * RB;
@@ -46,7 +40,7 @@ pack_x_kernel(const double* __restrict__ vvvo, int v, int vp, int o, int RB, TO*
         const size_t Rg = R0 + rr;
         const size_t db = Rg / v;
         const int c = (int)(Rg % v);
-        Splitter<TO>::put(X, Xlo, (size_t)k * plane + db * vp, c, tile[rr * op1 + k]);
+        X[(size_t)k * plane + db * vp + c] = operand_word<TO>(tile[rr * op1 + k]);
     }
 }
 
@@ -67,8 +61,7 @@ transpose_planes_kernel(const TO* __restrict__ X, int v, int vp, TO* __restrict_
 
 // Ot[r][p][a][l] = -ovoo[p][a][l][r]
 template <typename TO>
-__global__ void pack_ot_kernel(const double* __restrict__ ovoo, int v, int o, int op, TO* __restrict__ Ot,
-                               TO* __restrict__ Otlo) {
+__global__ void pack_ot_kernel(const double* __restrict__ ovoo, int v, int o, int op, TO* __restrict__ Ot) {
     const size_t n = (size_t)o * o * v * o;
     for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         const int l = (int)(e % o);
@@ -76,19 +69,18 @@ __global__ void pack_ot_kernel(const double* __restrict__ ovoo, int v, int o, in
         const int p = (int)((e / ((size_t)o * v)) % o);
         const int r = (int)(e / ((size_t)o * v * o));
         const double x = -ovoo[(((size_t)p * v + a) * o + l) * o + r];
-        Splitter<TO>::put(Ot, Otlo, (((size_t)r * o + p) * v + a) * op, l, x);
+        Ot[(((size_t)r * o + p) * v + a) * op + l] = operand_word<TO>(x);
     }
 }
 
 // T2[p][q][a][d] (d-pitch vp) = t2[p][q][a][d]
 template <typename TO>
-__global__ void pack_t2_kernel(const double* __restrict__ t2, size_t rows, int v, int vp, TO* __restrict__ T2,
-                               TO* __restrict__ T2lo) {
+__global__ void pack_t2_kernel(const double* __restrict__ t2, size_t rows, int v, int vp, TO* __restrict__ T2) {
     const size_t n = rows * v;
     for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         const size_t row = e / v;
         const int d = (int)(e % v);
-        Splitter<TO>::put(T2, T2lo, row * vp, d, t2[e]);
+        T2[row * vp + d] = operand_word<TO>(t2[e]);
     }
 }
 

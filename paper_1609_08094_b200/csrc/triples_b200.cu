@@ -246,19 +246,19 @@ int run_prepare_mixed(const Plan& P, const double* t2, const double* vvvo, const
         CU_TRY(cudaGetLastError());
         ++g_launches;
     }
-    pack_ot_kernel<float><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.ok, (float*)op.ot, nullptr);
+    pack_ot_kernel<float><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.ok, (float*)op.ot);
     CU_TRY(cudaGetLastError());
     ++g_launches;
-    pack_t2_kernel<float><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vk, (float*)op.t2, nullptr);
+    pack_t2_kernel<float><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vk, (float*)op.t2);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     return TRIPLES_OK;
 }
 
-template <typename TO>
 int run_prepare(const Plan& P, const double* t2, const double* vvvo, const double* ovoo, const Operands& op,
                 cudaStream_t st) {
     if (P.prec == TRIPLES_MIXED) return run_prepare_mixed(P, t2, vvvo, ovoo, op, st);
+    using TO = double;
     const int o = P.o, v = P.v;
     if (P.vp != v) {   // zero the pad columns (XT: entry c = v of a row is never written by the transpose)
         CU_TRY(cudaMemsetAsync(op.x, 0, P.n_x * sizeof(TO), st));
@@ -273,7 +273,7 @@ int run_prepare(const Plan& P, const double* t2, const double* vvvo, const doubl
         const size_t smem = (size_t)RB * (o + 1) * 8;
         auto kern = pack_x_kernel<TO>;
         CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
-        kern<<<(unsigned)((R + RB - 1) / RB), 256, smem, st>>>(vvvo, v, P.vp, o, RB, (TO*)op.x, nullptr);
+        kern<<<(unsigned)((R + RB - 1) / RB), 256, smem, st>>>(vvvo, v, P.vp, o, RB, (TO*)op.x);
         CU_TRY(cudaGetLastError());
         ++g_launches;
     }
@@ -287,10 +287,10 @@ int run_prepare(const Plan& P, const double* t2, const double* vvvo, const doubl
         }
         CU_TRY(cudaGetLastError());
     }
-    pack_ot_kernel<TO><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.op, (TO*)op.ot, nullptr);
+    pack_ot_kernel<TO><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.op, (TO*)op.ot);
     CU_TRY(cudaGetLastError());
     ++g_launches;
-    pack_t2_kernel<TO><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vp, (TO*)op.t2, nullptr);
+    pack_t2_kernel<TO><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vp, (TO*)op.t2);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     return TRIPLES_OK;
@@ -323,7 +323,7 @@ int run_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, c
         if (int rc = g_events.get(&ev_p1)) return rc;
         CU_TRY(cudaEventRecord(ev_p0, st));
     }
-    if (int rc = run_prepare<TS>(P, in.t2, in.vvvo, in.ovoo, op, st)) return rc;
+    if (int rc = run_prepare(P, in.t2, in.vvvo, in.ovoo, op, st)) return rc;
     if (prof) CU_TRY(cudaEventRecord(ev_p1, st));
 
     Maps maps;
@@ -628,7 +628,7 @@ int triples_w_block(int nocc, int nvirt, const double* t2, const double* vvvo, c
     uint8_t* ws = static_cast<uint8_t*>(workspace);
     Operands op = carve_operands(P, ws);
     g_launches = 0;
-    if (int rc = run_prepare<double>(P, t2, vvvo, ovoo, op, st)) return rc;
+    if (int rc = run_prepare(P, t2, vvvo, ovoo, op, st)) return rc;
     Maps maps;
     if (int rc = build_maps(P, op, &maps)) return rc;
     uint8_t* ubase = ws + P.off_u;
