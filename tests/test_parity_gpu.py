@@ -110,11 +110,12 @@ def test_tiny_config_large_t1_pins_e5():
 @pytest.mark.parametrize("o,v,naux,ijk", [
     (3, 5, 9, (0, 1, 2)), (3, 5, 9, (1, 1, 0)), (4, 17, 20, (3, 0, 2)), (5, 41, 50, (4, 2, 0)),
     (3, 50, 40, (0, 1, 2)), (6, 96, 60, (5, 1, 3)), (4, 130, 50, (1, 3, 2)), (8, 40, 120, (7, 3, 5)),
-    (17, 24, 30, (16, 0, 9)), (3, 258, 40, (2, 0, 1)), (35, 20, 40, (33, 0, 34)),
+    (17, 24, 30, (16, 0, 9)), (3, 258, 40, (2, 0, 1)), (35, 20, 40, (33, 0, 34)), (16, 160, 30, (5, 2, 11)),
 ])
 def test_w_block_elementwise_mixed(o, v, naux, ijk):
-    """FP32-accurate W: 3xTF32 products + FP32 accumulation of K = 2v + 2o terms, U stored in FP32.
-    Bound: (K rounding steps of the FP32 running sum + the split's 2^-21 cross term) on the scale of W."""
+    """FP32-class W: split products (TF32 main term, BF16 cross terms: 2^-12 * 2^-8 per product, Q13) +
+    FP32 accumulation of K = 2v + 2o terms in 2-chunk tensor-core chains, U stored in FP32.
+    Bound on the scale of W: cross-term rounding + truncation bias of the chains + FP32 running-sum rounding."""
     inp = synth.make_inputs(o, v, naux, seed=3)
     d = to_dev(inp)
     ws = workspace(o, v, tb.MIXED)
@@ -123,6 +124,9 @@ def test_w_block_elementwise_mixed(o, v, naux, ijk):
     Wo = oracle.w_block(o, v, inp.t2, inp.vvvo, inp.ovoo, *ijk)
     err = np.abs(W.cpu().numpy() - Wo).max()
     assert err <= 2e-6 * np.abs(Wo).max(), f"max abs err {err:.3e} vs scale {np.abs(Wo).max():.3e}"
+    # the chains' truncation bias (towards zero) stays below 1e-6 of W's own magnitude on average
+    Wg = W.cpu().numpy()
+    assert abs(np.sum(np.abs(Wg) - np.abs(Wo))) <= 1e-6 * np.sum(np.abs(Wo))
 
 
 @pytest.mark.parametrize("o,v,naux,t1_sigma", [
