@@ -35,7 +35,7 @@
 //                               TF32 MMAs (K = 8); tcgen05.commit multicasts to both CTAs' barriers)
 //   warps 2-7 : converters     (raw tile -> packed BF16 tile, ring of 2; warp 2 also allocates TMEM: 512 columns =
 //                               two 128 x 256 FP32 buffers in each CTA)
-//   warps 8-15: accumulators   (tcgen05.ld of every finished chain, FP32 round-to-nearest adds in registers,
+//   warps 8-15: accumulators   (tcgen05.ld of every finished chain, packed FP32 round-to-nearest adds (FADD2) in registers,
 //                               one 256-bit store per (b,c) row and a-tile of U at the end of the item)
 //
 // Why the running sum lives in registers and not in TMEM: the tensor core adds each MMA's result to its accumulator
@@ -272,9 +272,9 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
             int jb, rem;
             tf32_item(jobs, w, per_job, jb, rem);
             const int m0 = ((rem / ntiles) * cs + rank) * TF_BM, a0 = (rem % ntiles) * bn;
-            float acc[128];
+            uint64_t acc2[64];          // 128 FP32 running sums as 64 register pairs (packed add.rn.f32x2)
 #pragma unroll
-            for (int j = 0; j < 128; ++j) acc[j] = 0.0f;
+            for (int j = 0; j < 64; ++j) acc2[j] = 0ull;
             for (int ch = 0; ch < nchain; ++ch, ++chain) {
                 const uint32_t buf = chain & 1;
                 mbar_wait(&tfull[buf], (chain >> 1) & 1);
@@ -287,7 +287,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                         tmem_ld_32x32b_x16(taddr + c0, rg);
                         tmem_ld_wait();
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) acc[c0 + j] = __fadd_rn(acc[c0 + j], __uint_as_float(rg[j]));
+                        for (int j = 0; j < 8; ++j) acc2[c0 / 2 + j] = fadd2_rn(acc2[c0 / 2 + j], rg[2 * j], rg[2 * j + 1]);
                     }
                 }
                 tc_fence_before_sync();
@@ -313,11 +313,13 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
 #pragma unroll
                 for (int t = 0; t < 16; ++t) {
                     if (8 * t < acols) {
-                        float u[8], w[8];
+                        float acc[8], u[8], w[8];        // the tile's 8 columns, unpacked
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) unpack_f32x2(acc2[4 * t + j], acc[2 * j], acc[2 * j + 1]);
 #pragma unroll
                         for (int j = 0; j < 4; ++j) {
-                            u[j] = s4 ? acc[8 * t + j + 4] : acc[8 * t + j];
-                            u[j + 4] = s4 ? acc[8 * t + j] : acc[8 * t + j + 4];
+                            u[j] = s4 ? acc[j + 4] : acc[j];
+                            u[j + 4] = s4 ? acc[j] : acc[j + 4];
                         }
 #pragma unroll
                         for (int j = 0; j < 8; ++j) w[j] = s2 ? u[j ^ 2] : u[j];

@@ -183,6 +183,17 @@ __device__ __forceinline__ void tmem_ld_32x32b_x16(uint32_t taddr, uint32_t (&r)
         : "memory");
 }
 // Register re-partitioning between warpgroups (all four warps of a warpgroup execute the same instruction).
+// packed FP32 add (sm_100: FADD2), round to nearest: (acc.lo + a, acc.hi + b)
+__device__ __forceinline__ uint64_t fadd2_rn(uint64_t acc, uint32_t a, uint32_t b) {
+    uint64_t r;
+    asm("{\n\t.reg .b64 t;\n\tmov.b64 t, {%2, %3};\n\tadd.rn.f32x2 %0, %1, t;\n\t}" : "=l"(r) : "l"(acc), "r"(a), "r"(b));
+    return r;
+}
+__device__ __forceinline__ void unpack_f32x2(uint64_t v, float& lo, float& hi) {
+    uint32_t a, b;
+    asm("mov.b64 {%0, %1}, %2;" : "=r"(a), "=r"(b) : "l"(v));
+    lo = __uint_as_float(a); hi = __uint_as_float(b);
+}
 // 256-bit global store (sm_100: STG.256), 32-byte aligned
 __device__ __forceinline__ void stg_v8(float* p, const float (&w)[8]) {
     asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(w[0]), "f"(w[1]), "f"(w[2]), "f"(w[3]),
