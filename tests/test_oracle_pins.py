@@ -324,3 +324,34 @@ def test_generator_preconditions():
     assert np.allclose(inp.ovov, inp.ovov.transpose(2, 3, 0, 1), atol=1e-14)       # (ia|jb) = (jb|ia)
     for arr in inp.arrays():
         assert arr.dtype == np.float64 and arr.flags.c_contiguous
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# regression goldens (tests/golden/oracle_energies.json, written by tests/golden/make_golden.py from the oracle only;
+# absolute values are "parity unpinned by the paper", DESIGN.md section 4 P10)
+# ------------------------------------------------------------------------------------------------------------------
+def _golden():
+    import json
+    import os
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_energies.json")) as f:
+        return json.load(f)
+
+
+def test_oracle_reproduces_its_golden_values_tiny():
+    g = _golden()["tiny"]
+    inp = synth.make_config("tiny", seed=0)
+    E, et = oracle.energy_restricted(inp.nocc, inp.nvirt, *inp.arrays(), with_triplets=True)
+    assert np.allclose(E, g["E"], rtol=1e-13, atol=0.0)
+    assert np.allclose(et, np.array(g["triplets"]), rtol=1e-12, atol=1e-18)
+    # Q1: the (T) correction is negative; E[4] <= 0 triplet by triplet (P6)
+    assert g["E"][0] < 0 and np.all(np.array(g["triplets"])[:, 1] <= 0)
+
+
+def test_numpy_restatement_reproduces_its_golden_values_small():
+    g = _golden()["small"]
+    inp = synth.make_config("small", seed=0)
+    a = inp.arrays()
+    pick = [1, 3, 7]
+    trips = [tuple(g["triplets_ijk"][n]) for n in pick]
+    e = oracle.energy_subset_numpy(a[0], a[1], a[2], a[3], a[4], a[5], a[6], trips)
+    assert np.allclose(e, np.array(g["energies"])[pick], rtol=1e-12, atol=0.0)

@@ -331,3 +331,46 @@ def test_profile_and_launch_count():
     assert p["contraction_flops"] == pytest.approx((T - o) * full - n_pair * full / 3, rel=1e-12)
     assert p["contraction_ms"] > 0 and p["reduction_ms"] > 0
     assert tb.triples_last_launch_count() >= 3 * p["contraction_launches"] + 1
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# stored oracle values (tests/golden/, written by a script that calls only oracle/): no oracle run needed here
+# ------------------------------------------------------------------------------------------------------------------
+def _golden():
+    import json
+    import os
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_energies.json")) as f:
+        return json.load(f)
+
+
+@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED], ids=["fp64", "mixed"])
+def test_tiny_config_against_golden(prec):
+    g = _golden()["tiny"]
+    inp = synth.make_config("tiny", seed=0)
+    (E, et) = gpu_energy(inp, prec=prec, with_triplets=True)
+    for n in range(2):
+        assert rel(E[n], g["E"][n]) <= TOL[prec], (n, E, g["E"])
+    assert abs(E[2] - g["E"][2]) <= TOL[prec] * max(abs(g["E"][2]), 1e-3 * abs(g["E"][1]))
+    got, want = et, np.array(g["triplets"])
+    assert np.abs(got[:, :2] - want[:, :2]).max() <= TOL[prec] * np.abs(want[:, 1]).max()
+
+
+@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED], ids=["fp64", "mixed"])
+@pytest.mark.parametrize("name", ["small", "medium"])
+def test_sampled_triplets_against_golden(name, prec):
+    g = _golden()[name]
+    inp = synth.make_config(name, seed=0)
+    o, v = inp.nocc, inp.nvirt
+    assert (o, v) == (g["nocc"], g["nvirt"])
+    d = to_dev(inp)
+    trips = [tuple(t) for t in g["triplets_ijk"]]
+    e_gpu = tb.triples_energy_subset(o, v, *d, prec, trips, workspace(o, v, prec))
+    want = np.array(g["energies"])
+    for n, t in enumerate(trips):
+        if t[0] == t[1] == t[2]:
+            assert np.all(e_gpu[n] == 0.0) and np.abs(want[n]).max() <= 1e-12 * np.abs(want[:, 1]).max()
+            continue
+        s4 = abs(want[n, 1])
+        assert abs(e_gpu[n, 0] - want[n, 0]) <= TOL[prec] * s4, (t, e_gpu[n], want[n])
+        assert abs(e_gpu[n, 1] - want[n, 1]) <= TOL[prec] * s4, (t, e_gpu[n], want[n])
+        assert abs(e_gpu[n, 2] - want[n, 2]) <= max(TOL[prec] * s4, 100 * TOL[prec] * abs(want[n, 2])), (t, e_gpu[n], want[n])
