@@ -1,0 +1,92 @@
+"""Host-side logic of bench.py (no GPU): the rank reduction used for multi-process runs (world size 2, gloo, CPU),
+the flop formula of the metric, and the reference arm (the CPU oracle timed on a bounded sample)."""
+import json
+import os
+import socket
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+import bench  # noqa: E402
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, {root!r})
+import torch.distributed as dist
+import bench
+dist.init_process_group("gloo")
+rank = dist.get_rank()
+t, u = bench.reduce_over_ranks(1.0 + rank, 10.0 * (rank + 1), dist.get_world_size())
+print(json.dumps({{"rank": rank, "t": t, "u": u}}), flush=True)
+dist.destroy_process_group()
+"""
+
+
+def test_reduce_over_ranks_world_size_2_gloo():
+    """Replicas-only multi-GPU path: MAX of the per-rank times, SUM of the per-rank units."""
+    port = _free_port()
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, "-c", _WORKER.format(root=ROOT)], env=env,
+                                      stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    outs = []
+    for p in procs:
+        out, err = p.communicate(timeout=180)
+        assert p.returncode == 0, err[-2000:]
+        outs.append(json.loads(out.strip().splitlines()[-1]))
+    for o in outs:
+        assert o["t"] == 2.0 and o["u"] == 30.0       # max(1, 2) seconds, 10 + 20 units on every rank
+
+
+def test_reduce_over_ranks_single_process_is_identity():
+    assert bench.reduce_over_ranks(1.5, 7.0, 1) == (1.5, 7.0)
+
+
+@pytest.mark.parametrize("o,v", [(8, 40), (24, 240), (40, 480)])
+def test_formula_flops_is_the_papers_task_count_times_the_gemm_flops(o, v):
+    # PAPER.md Eq. (5.0.7b): T = No(No+1)(No+2)/6 equal-weight tasks; 12 v^4 + 12 o v^3 flop each
+    T = sum((o - i) * (1 + (o - i)) // 2 for i in range(o))
+    assert bench.formula_flops(o, v) == T * (12.0 * v ** 4 + 12.0 * o * v ** 3)
+
+
+def test_measured_peaks_has_the_roofline_denominators():
+    peaks, kind = bench.measured_peaks()
+    assert kind in ("measured", "fallback")
+    assert peaks["hbm_gbs"] > 1000 and peaks["bf16_tflops_sustained"] > 100
+
+
+def _run_reference(extra_env):
+    env = dict(os.environ, **extra_env)
+    return subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "tiny",
+                           "--steps", "1", "--warmup", "1", "--ref-triplets", "2"], env=env, capture_output=True,
+                          text=True, timeout=600)
+
+
+def test_reference_arm_times_the_oracle_and_prints_one_json_line():
+    res = _run_reference({})
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [ln for ln in res.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["unit"] == "TFLOP/s" and d["higher_is_better"] is True
+    assert d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
+    assert d["e2e"] == {"value": d["value"], "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert d["gpu_launches"] == 0 and "tiny" in d["config"]["workload"]
+
+
+def test_reference_arm_other_ranks_exit_quietly():
+    res = _run_reference({"RANK": "1", "WORLD_SIZE": "2", "LOCAL_RANK": "1"})
+    assert res.returncode == 0 and res.stdout.strip() == ""
