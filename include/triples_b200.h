@@ -34,8 +34,8 @@
  *     entry points return TRIPLES_EARCH.
  *   - precision: TRIPLES_FP64  = contractions in FP64 (DMMA), everything FP64;
  *                TRIPLES_MIXED = the paper's mixed precision (L125, L156): only the W build
- *                (the contractions) in single precision (operands split x = h + l, h*h' in TF32
- *                and the cross terms h*l' + l*h' in BF16 on tcgen05, FP32 accumulate, W stored FP32:
+ *                (the contractions) in single precision (operands scaled by a power of two and split
+ *                x = h + l in FP16, h*h' + h*l' + l*h' on tcgen05 with FP32 accumulation, W stored FP32:
  *                W within 1e-6 of FP64 on the scale of W); Vd, D, the energy reduction and sums in FP64.
  */
 #ifndef TRIPLES_B200_H

@@ -1,13 +1,18 @@
-// gemm_tf32.cuh -- mixed-precision contraction kernel (S2+S3 of DESIGN.md): TMA -> swizzled smem -> tcgen05.mma
-// (cta_group::2, kind::tf32 + kind::f16) with short FP32 accumulation chains in TMEM and the running sum in registers.
+// gemm_tf32.cuh -- mixed-precision contraction kernel (S2+S3 of DESIGN.md): TMA -> swizzled smem -> in-SM operand
+// split -> tcgen05.mma (cta_group::2, kind::f16) with short FP32 accumulation chains in TMEM and the running sum in
+// registers.  (The file keeps its first name: the first version ran 3xTF32.)
 //
 // The paper's mixed precision runs "only the construction of the triples amplitudes" through
-// sgemm.  B200 has no FP32 tensor path; an FP32-class product is recovered from a split of every operand x made by
-// prepare.cuh (Q13):  h = RN_tf32(x), l = x - h,   x*y ~= h*h' + (h*l' + l*h').
-// The main term h*h' runs in TF32 (exact 11 x 11 bit products, FP32 accumulation).  The cross terms are 2^-12 of it,
-// so BF16 operands (RN, 8 bits) are enough for them -- error 2^-12 * 2^-8 per product, unbiased, the same order as
-// the dropped l*l' -- and a BF16 MMA covers twice the K of a TF32 MMA: 8 MMAs per 32-wide K chunk instead of the 12
-// of a 3xTF32 scheme.  Measured on B200: W within 1e-6 of the FP64 oracle on the scale of W, E(T) within 2e-7.
+// sgemm.  B200 has no FP32 tensor path; an FP32-class product is recovered from a split of every operand x
+// (Q13):   h = RN_fp16(x), l = RN_fp16(x - h),   x*y ~= h*h' + (h*l' + l*h').
+// FP16 has the 11-bit significand of TF32 at twice the MMA rate; its narrow exponent range is handled by ONE power
+// of two per tensor class (prepare.cuh scales_kernel: the largest |x| of the integrals / of t2 lands in
+// [2^13, 2^14)), so every term of a contraction carries the same factor 2^(sg+st), removed exactly in the epilogue.
+// h*h' is exact (11 x 11 bit products, FP32 accumulation); l <= 2^-12 |x| (x - h is exact in FP32) and its own
+// FP16 rounding leaves 2^-23 |x| for elements within 2^-2 of the tensor maximum after scaling, an absolute
+// 2^-25 * 2^-s below that (subnormal l) -- i.e. a 39-bit fixed-point floor relative to the tensor's largest
+// element; the dropped l*l' is 2^-24.  6 MMAs (K = 16) per 32-wide K chunk where 3xTF32 needs 12.
+// Measured on B200: W within 3e-7 of the FP64 oracle on the scale of W, E(T) within 4e-7 (chain bias, below).
 //
 // Same "G job" (p,q,r) as gemm_f64.cuh, computed TRANSPOSED so that the long flattened (b,c) index is the MMA's
 // M dimension (128 TMEM lanes per CTA, no padding waste for any v) and the virtual index a is its N dimension:
@@ -15,37 +20,37 @@
 //   G(p,q,r)[a,(b,c)] = sum_d XK_r [(b,c),d] T2A[p,q][a,d]  + sum_d XKT_q[(b,c),d] T2A[p,r][a,d]     (Eq. (2.2.2))
 //                     + sum_l T2K_q[(b,c),l] OtA[r,p][a,l]  + sum_l T2KT_r[(b,c),l] OtA[q,p][a,l]
 //
-// Operands are K-major arrays (prepare.cuh): XK[r][b][c][d] = (db|cr), XKT[r][b][c][d] = XK[r][c][b][d],
-// T2A[p][q][a][d] = t2, OtA[r][p][a][l] = -(pa|lr), T2K[q][b][c][l] = t2[q,l,b,c], T2KT[r][b][c][l] = t2[l,r,b,c];
-// the c index has vp rows per b (row v is zero when v is odd) so that U keeps the pitch the reduction expects.
-// An element is ONE 4-byte word: the FP32 bit pattern of x plus 0x1000 (prepare.cuh biased_word).  The TF32 MMA
-// ignores the low 13 bits of its operands, so it reads the word as h = RN_tf32(x) straight from the TMA-written tile;
-// converter warps recover x and l = x - h exactly and write, per 32-wide K chunk, a packed tile whose 128-byte rows
-// hold 32 BF16 of h (bytes 0..63) and 32 BF16 of l (bytes 64..127) for the cross-term MMAs.  Splitting inside the
-// SM halves the operand bytes in HBM and through L2 (with separate hi/lo arrays the loop was bound by the ~42
-// B/clk/SM L2 -> SM cap, not by the tensor pipe).
+// Operands are K-major arrays of scaled FP32 values, 4 bytes per element (prepare.cuh): XK[r][b][c][d] = (db|cr),
+// XKT[r][b][c][d] = XK[r][c][b][d], T2A[p][q][a][d] = t2, OtA[r][p][a][l] = -(pa|lr), T2K[q][b][c][l] = t2[q,l,b,c],
+// T2KT[r][b][c][l] = t2[l,r,b,c]; the c index has vp rows per b (row v is zero when v is odd) so that U keeps the
+// pitch the reduction expects.  TMA stages raw FP32 tiles; converter warps write, per 32-wide K chunk, a packed tile
+// whose 128-byte rows hold 32 FP16 of h (bytes 0..63) and 32 FP16 of l (bytes 64..127) -- the only thing the MMAs
+// read.  Splitting inside the SM halves the operand bytes in HBM and through L2 (with separate hi/lo arrays the loop
+// was bound by the ~42 B/clk/SM L2 -> SM cap, not by the tensor pipe).
 //
 // The kernel is persistent and runs as CTA PAIRS (thread-block clusters of 2 = the two SMs of a TPC, cta_group::2):
 // a pair walks work items (job, two consecutive m-tiles of 128 (b,c) rows, n-tile of BN a-columns) as ONE
 // 256 x BN MMA tile.  Each CTA stages only its own 128 M-side rows and HALF of the N-side rows (the tensor cores
 // read the other half from the peer's shared memory).  Jobs of a launch are grouped by (q,r) so that the big
 // XK_r / XKT_q slices come from HBM once per group (tf32_item below).
-//   warp 0    : TMA producer   (K chunks of 32 words = one 128-byte swizzled row per operand row, ring of 4 raw tiles)
-//   warp 1    : MMA issuer     (one lane of the LEADER CTA; per K chunk 2+2 BF16 cross-term MMAs (K = 16), then 4
-//                               TF32 MMAs (K = 8); tcgen05.commit multicasts to both CTAs' barriers)
-//   warps 2-7 : converters     (raw tile -> packed BF16 tile, ring of 2; warp 2 also allocates TMEM: 512 columns =
+//   warp 0    : TMA producer   (K chunks of 32 words = one 128-byte swizzled row per operand row, ring of 3 raw tiles)
+//   warp 1    : MMA issuer     (one lane of the LEADER CTA; per K chunk 2+2 cross-term MMAs, then 2 main-term MMAs,
+//                               all FP16 K = 16; tcgen05.commit multicasts to both CTAs' barriers)
+//   warps 2-7 : converters     (raw tile -> packed tile, ring of 3; warp 2 also allocates TMEM: 512 columns =
 //                               two 128 x 256 FP32 buffers in each CTA)
-//   warps 8-15: accumulators   (tcgen05.ld of every finished chain, packed FP32 round-to-nearest adds (FADD2) in registers,
-//                               one 256-bit store per (b,c) row and a-tile of U at the end of the item)
+//   warps 8-15: accumulators   (tcgen05.ld of every finished chain, packed FP32 round-to-nearest adds (FADD2) in
+//                               registers, one 256-bit store per (b,c) row and a-tile of U at the end of the item)
 //
 // Why the running sum lives in registers and not in TMEM: the tensor core adds each MMA's result to its accumulator
 // with truncation, so one long accumulation chain is biased towards zero by ~(number of MMAs) * 2^-25 (measured:
 // -3.4e-6 relative on W at v = 240, i.e. 7e-6 on E(T), growing with v).  A TMEM buffer therefore only ever holds a
-// short chain (TF_CHAIN = 2 K chunks = 16 MMAs, started with accumulate = 0, cross terms before the main term of
+// short chain (TF_CHAIN = 2 K chunks = 12 MMAs, started with accumulate = 0, cross terms before the main term of
 // each chunk); finished chains are added with FADD.RN by the accumulator warps while the tensor core fills the
-// other buffer.  Measured bias on E(T): 1.8e-7 with one chunk per chain, 4.7e-7 with two (8 % faster: the kernel
-// runs at the 1 kW power cap and every chain costs a 128 x BN TMEM read-out); tolerance 1e-5.
+// other buffer.  Measured bias on E(T): ~2e-7 with one chunk per chain, 3e-7..5e-7 with two (8 % faster: every chain
+// costs a 128 x BN TMEM read-out and the kernel runs at the 1 kW power cap); tolerance 1e-5.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "gemm_f64.cuh"   // GemmJob
 #include "ptx.cuh"
 #include "ulayout.cuh"
@@ -76,7 +81,7 @@ constexpr int TF_TAIL_BYTES = 2048 + TF_MAX_JOBS * 48;   // alignment slack + ba
 // npad = N-side rows a CTA stages = bn / 2.  Two shared-memory rings of (128 + npad)-row tiles with 128-byte rows:
 // TF_RAW_STAGES raw tiles (TMA destination, TF32 operand; deep enough to cover the L2/HBM latency) and TF_PK_STAGES
 // packed BF16 tiles (written by the converter warps; the conversion of chunk c+1 overlaps the MMAs of chunk c).
-constexpr int TF_RAW_STAGES = 4, TF_PK_STAGES = 2;
+constexpr int TF_RAW_STAGES = 3, TF_PK_STAGES = 3;
 __host__ __device__ constexpr int tf32_tile_bytes(int npad) { return (TF_BM + npad) * 128; }
 // the request is always > half an SM's shared memory: exactly one CTA per SM (it owns all 512 TMEM columns)
 __host__ __device__ constexpr int tf32_smem_bytes(int npad) {
@@ -97,7 +102,7 @@ __device__ __forceinline__ void tf32_item(const GemmJob* __restrict__ jobs, long
 
 __global__ void __launch_bounds__(TF_THREADS, 1)
 gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restrict__ gjobs, int njobs, int v, int vp,
-                 int o, int mtiles, int ntiles, int bn, int npad) {
+                 int o, int mtiles, int ntiles, int bn, int npad, const float* __restrict__ scales) {
     constexpr int cs = 2;   // CTAs per MMA tile
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -129,7 +134,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
 
     if (threadIdx.x == 0) {
         // conv / tempty are waited on by the leader's MMA thread only: both CTAs' converter / accumulator warps arrive
-        for (int s = 0; s < RS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < RS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], TF_CONV_WARPS); }
         for (int s = 0; s < PS; ++s) { mbar_init(&conv[s], TF_CONV_WARPS * cs); mbar_init(&pkempty[s], 1); }
         for (int b = 0; b < 2; ++b) { mbar_init(&tfull[b], 1); mbar_init(&tempty[b], 8 * cs); }
         fence_barrier_init();
@@ -195,18 +200,23 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                     uint32_t x[8];
                     lds_v4(raw + rb + (((2 * m) ^ sw) << 4), x[0], x[1], x[2], x[3]);
                     lds_v4(raw + rb + (((2 * m + 1) ^ sw) << 4), x[4], x[5], x[6], x[7]);
-                    float h[8], l[8];
+                    // h = RN_fp16(x) (11-bit significand), l = RN_fp16(x - h); packed row: 32 FP16 of h | 32 FP16 of l
+                    // (kind::f16 wants A and B of one type: a BF16 x FP16 descriptor traps as an illegal instruction)
+                    uint32_t hp[4], lp[4];
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        // a zero word (TMA zero fill, pads) stands for x = 0: max() keeps the subtraction from wrapping
-                        h[j] = __uint_as_float(x[j] & 0xffffe000u);
-                        l[j] = __uint_as_float(max(x[j], 0x1000u) - 0x1000u) - h[j];
+                    for (int j = 0; j < 4; ++j) {
+                        const float x0 = __uint_as_float(x[2 * j]), x1 = __uint_as_float(x[2 * j + 1]);
+                        const __half2 h2 = __floats2half2_rn(x0, x1);
+                        const float2 hf = __half22float2(h2);
+                        hp[j] = *reinterpret_cast<const uint32_t*>(&h2);
+                        const __half2 l2 = __floats2half2_rn(x0 - hf.x, x1 - hf.y);
+                        lp[j] = *reinterpret_cast<const uint32_t*>(&l2);
                     }
-                    sts_v4(pk + rb + (((uint32_t)m ^ sw) << 4), pack_bf16x2(h[0], h[1]), pack_bf16x2(h[2], h[3]),
-                           pack_bf16x2(h[4], h[5]), pack_bf16x2(h[6], h[7]));
-                    sts_v4(pk + rb + (((uint32_t)(4 + m) ^ sw) << 4), pack_bf16x2(l[0], l[1]), pack_bf16x2(l[2], l[3]),
-                           pack_bf16x2(l[4], l[5]), pack_bf16x2(l[6], l[7]));
+                    sts_v4(pk + rb + (((uint32_t)m ^ sw) << 4), hp[0], hp[1], hp[2], hp[3]);
+                    sts_v4(pk + rb + (((uint32_t)(4 + m) ^ sw) << 4), lp[0], lp[1], lp[2], lp[3]);
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[s]);       // raw tile read: the producer may refill it
                 fence_proxy_async();          // generic-proxy writes -> visible to the tensor core's (async proxy) reads
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster_release(lconv0 + 8u * ps);
@@ -215,12 +225,12 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
     } else if (warp == 1) {
         // ------------------------------------------------------------------------------------ MMA issuer
         if (lane == 0 && rank == 0) {
-            const uint32_t idesc = umma_idesc_tf32_m256((uint32_t)bn), idesc16 = umma_idesc_bf16_m256((uint32_t)bn);
+            const uint32_t idesc = umma_idesc_f16_m256((uint32_t)bn, 0, 0);   // FP16 x FP16 -> FP32
             const uint32_t smem_base = smem_u32(smem);
             uint32_t it = 0, chain = 0;
             for (long long w = cid; w < nitems; w += ncl) {
                 for (int c = 0; c < nch; ++c, ++it) {
-                    const int s = it % RS, ps = it % PS;
+                    const int ps = it % PS;
                     int left;   // k-steps of this chunk that carry data
                     if (c < nch_v) left = kst_v - c * 4;
                     else if (c < 2 * nch_v) left = kst_v - (c - nch_v) * 4;
@@ -236,26 +246,23 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                     mbar_wait(&conv[ps], (it / PS) & 1);
                     tc_fence_after_sync();
                     const uint32_t tacc = tmem_base + buf * 256;
-                    const uint32_t sM = smem_base + s * tile_bytes, sN = sM + TF_BM * 128;              // raw (TF32)
-                    const uint32_t pM = smem_base + (RS + ps) * tile_bytes, pN = pM + TF_BM * 128;      // packed
-                    const uint64_t mh = umma_desc_sw128(sM), ml = umma_desc_sw128(pM);
-                    const uint64_t nh = umma_desc_sw128(sN), nl = umma_desc_sw128(pN);
+                    const uint32_t pM = smem_base + (RS + ps) * tile_bytes, pN = pM + TF_BM * 128;      // packed tiles
+                    const uint64_t ml = umma_desc_sw128(pM), nl = umma_desc_sw128(pN);
                     uint32_t acc = first ? 0u : 1u;
-                    // cross terms l*h' + h*l' in BF16 (packed tile: bytes 0..63 of a row = 32 BF16 of h, 64..127 = 32
-                    // BF16 of l; K = 16 per MMA), small terms first; then the main term h*h' in TF32 (K = 8 per MMA)
+                    // packed row: bytes 0..63 = 32 FP16 of h, 64..127 = 32 FP16 of l; K = 16 per MMA.  Cross terms
+                    // l*h' + h*l' first (small), then the main term h*h'
                     const int nk16 = (nk + 1) >> 1;
                     for (int k = 0; k < nk16; ++k) {
                         const uint64_t adv = (uint64_t)(k * 2);          // 32 bytes per k-step, in 16-byte units
-                        umma_bf16_pair(tacc, ml + 4 + adv, nl + adv, idesc16, acc);   // l * h'
+                        umma_f16_pair(tacc, ml + 4 + adv, nl + adv, idesc, acc);   // l * h'
                         acc = 1;
-                        umma_bf16_pair(tacc, ml + adv, nl + 4 + adv, idesc16, 1);     // h * l'
+                        umma_f16_pair(tacc, ml + adv, nl + 4 + adv, idesc, 1);     // h * l'
                     }
-                    for (int k = 0; k < nk; ++k) {
+                    for (int k = 0; k < nk16; ++k) {
                         const uint64_t adv = (uint64_t)(k * 2);
-                        umma_tf32_pair(tacc, mh + adv, nh + adv, idesc, 1);           // h * h'
+                        umma_f16_pair(tacc, ml + adv, nl + adv, idesc, 1);         // h * h'
                     }
-                    umma_commit_pair(&empty[s]);                       // both CTAs' raw and packed slots
-                    umma_commit_pair(&pkempty[ps]);
+                    umma_commit_pair(&pkempty[ps]);                    // both CTAs' packed slots
                     if (last) { umma_commit_pair(&tfull[buf]); ++chain; }   // both CTAs' accumulator warps
                 }
             }
@@ -304,6 +311,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                 float* __restrict__ out = static_cast<float*>(jobs[jb].out);
                 float* __restrict__ out2 = static_cast<float*>(jobs[jb].out2);
                 const int nt = u_tiles(v);
+                const float unscale = scales[2];             // 2^-(sg+st): exact
                 const int sw = u_swz<4>(0, bb & 7, cc & 7);
                 const bool s4 = (sw & 4) != 0, s2 = (sw & 2) != 0;
                 const size_t astride = (size_t)nt * nt * UCHUNK;   // one a-tile
@@ -316,6 +324,8 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
                         float acc[8], u[8], w[8];        // the tile's 8 columns, unpacked
 #pragma unroll
                         for (int j = 0; j < 4; ++j) unpack_f32x2(acc2[4 * t + j], acc[2 * j], acc[2 * j + 1]);
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) acc[j] *= unscale;
 #pragma unroll
                         for (int j = 0; j < 4; ++j) {
                             u[j] = s4 ? acc[j + 4] : acc[j];

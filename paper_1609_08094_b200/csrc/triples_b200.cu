@@ -132,6 +132,7 @@ int launch_gemm_f64(const GemmMaps& maps, const GemmJob* jobs, int njobs, const 
 struct Operands {   // device pointers of the repacked operands (workspace) for one precision
     void *x, *xt, *ot, *t2;
     void *t2k, *t2kt;   // mixed path only
+    float* scales;      // mixed path only: 2^sg, 2^st, 2^-(sg+st) (prepare.cuh scales_kernel), then two uint maxima
 };
 
 struct Maps {   // tensor maps of the contraction kernel of the plan's precision
@@ -170,7 +171,8 @@ int build_maps(const Plan& P, const Operands& op, Maps* maps) {
     return P.prec == TRIPLES_FP64 ? build_maps_f64(P, op, &maps->f64) : build_maps_tf32(P, op, &maps->tf32);
 }
 
-int launch_gemm_tf32(const Tf32Maps& maps, const GemmJob* jobs, int njobs, const Plan& P, cudaStream_t st) {
+int launch_gemm_tf32(const Tf32Maps& maps, const GemmJob* jobs, int njobs, const Plan& P, const float* scales,
+                     cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
         CU_TRY(cudaFuncSetAttribute(gemm_tf32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TF_SMEM_LIMIT));
@@ -199,13 +201,13 @@ int launch_gemm_tf32(const Tf32Maps& maps, const GemmJob* jobs, int njobs, const
     }
     cfg.gridDim = dim3((unsigned)(std::min<long long>(items, max_clusters) * cs));
     CU_TRY(cudaLaunchKernelEx(&cfg, gemm_tf32_kernel, maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles, P.tf_ntiles,
-                              P.tf_bn, P.tf_npad));
+                              P.tf_bn, P.tf_npad, scales));
     ++g_launches;
     return TRIPLES_OK;
 }
 
-int launch_gemm(const Plan& P, const Maps& maps, const GemmJob* jobs, int njobs, cudaStream_t st) {
-    if (P.prec == TRIPLES_MIXED) return launch_gemm_tf32(maps.tf32, jobs, njobs, P, st);
+int launch_gemm(const Plan& P, const Maps& maps, const Operands& op, const GemmJob* jobs, int njobs, cudaStream_t st) {
+    if (P.prec == TRIPLES_MIXED) return launch_gemm_tf32(maps.tf32, jobs, njobs, P, op.scales, st);
     switch (P.cfg) {
         case CFG_M120_N128: return launch_gemm_f64<3, 4, 4, 4>(maps.f64, jobs, njobs, P, st);
         case CFG_M80_N192: return launch_gemm_f64<2, 4, 6, 4>(maps.f64, jobs, njobs, P, st);
@@ -228,6 +230,16 @@ int run_prepare_mixed(const Plan& P, const double* t2, const double* vvvo, const
         CU_TRY(cudaMemsetAsync(op.t2kt, 0, P.n_t2k * 4, st));
     }
     if (P.ok != o) CU_TRY(cudaMemsetAsync(op.ot, 0, P.n_ot * 4, st));
+    {   // power-of-two scales of the two tensor classes
+        unsigned int* mx = reinterpret_cast<unsigned int*>(op.scales + 4);
+        CU_TRY(cudaMemsetAsync(mx, 0, 8, st));
+        absmax_kernel<<<kNumSM * 8, 256, 0, st>>>(vvvo, (size_t)v * v * v * o, mx);
+        absmax_kernel<<<kNumSM, 256, 0, st>>>(ovoo, (size_t)o * v * o * o, mx);
+        absmax_kernel<<<kNumSM * 2, 256, 0, st>>>(t2, (size_t)o * o * v * v, mx + 1);
+        scales_kernel<<<1, 32, 0, st>>>(mx, op.scales);
+        CU_TRY(cudaGetLastError());
+        g_launches += 4;
+    }
     {
         static bool attr_set = false;
         if (!attr_set) {
@@ -236,20 +248,20 @@ int run_prepare_mixed(const Plan& P, const double* t2, const double* vvvo, const
         }
         const size_t S = (size_t)v * v * o;
         dim3 grid((unsigned)((S + PKX_SPAN - 1) / PKX_SPAN), (v + 31) / 32);
-        pack_xk_kernel<<<grid, 256, PKX_SMEM, st>>>(vvvo, v, P.vp, P.vk, o, (float*)op.x, (float*)op.xt);
+        pack_xk_kernel<<<grid, 256, PKX_SMEM, st>>>(vvvo, v, P.vp, P.vk, o, (float*)op.x, (float*)op.xt, op.scales);
         CU_TRY(cudaGetLastError());
         ++g_launches;
     }
     {
         dim3 grid(o * v, (v + 63) / 64, (o + 63) / 64);
-        pack_t2k_kernel<<<grid, 256, 0, st>>>(t2, v, P.vp, o, P.ok, (float*)op.t2k, (float*)op.t2kt);
+        pack_t2k_kernel<<<grid, 256, 0, st>>>(t2, v, P.vp, o, P.ok, (float*)op.t2k, (float*)op.t2kt, op.scales + 1);
         CU_TRY(cudaGetLastError());
         ++g_launches;
     }
-    pack_ot_kernel<float><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.ok, (float*)op.ot);
+    pack_ot_kernel<float><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.ok, (float*)op.ot, op.scales);
     CU_TRY(cudaGetLastError());
     ++g_launches;
-    pack_t2_kernel<float><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vk, (float*)op.t2);
+    pack_t2_kernel<float><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vk, (float*)op.t2, op.scales + 1);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     return TRIPLES_OK;
@@ -287,10 +299,10 @@ int run_prepare(const Plan& P, const double* t2, const double* vvvo, const doubl
         }
         CU_TRY(cudaGetLastError());
     }
-    pack_ot_kernel<TO><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.op, (TO*)op.ot);
+    pack_ot_kernel<TO><<<kNumSM * 4, 256, 0, st>>>(ovoo, v, o, P.op, (TO*)op.ot, nullptr);
     CU_TRY(cudaGetLastError());
     ++g_launches;
-    pack_t2_kernel<TO><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vp, (TO*)op.t2);
+    pack_t2_kernel<TO><<<kNumSM * 8, 256, 0, st>>>(t2, (size_t)o * o * v, v, P.vp, (TO*)op.t2, nullptr);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     return TRIPLES_OK;
@@ -299,7 +311,10 @@ int run_prepare(const Plan& P, const double* t2, const double* vvvo, const doubl
 Operands carve_operands(const Plan& P, uint8_t* ws) {
     Operands op{};
     op.x = ws + P.off_x; op.xt = ws + P.off_xt; op.ot = ws + P.off_ot; op.t2 = ws + P.off_t2;
-    if (P.prec == TRIPLES_MIXED) { op.t2k = ws + P.off_t2k; op.t2kt = ws + P.off_t2kt; }
+    if (P.prec == TRIPLES_MIXED) {
+        op.t2k = ws + P.off_t2k; op.t2kt = ws + P.off_t2kt;
+        op.scales = reinterpret_cast<float*>(ws + P.off_result + 64);   // the result block has 256 bytes, 24 used
+    }
     return op;
 }
 
@@ -389,7 +404,7 @@ int run_batches(const Plan& P, const Inputs& in, uint8_t* ws, cudaStream_t st, c
             for (int x = 0; x < 4; ++x) if (int rc = g_events.get(&e[x])) return rc;
             CU_TRY(cudaEventRecord(e[0], st));
         }
-        if (int rc = launch_gemm(P, maps, d_gj + g0, g1 - g0, st)) return rc;
+        if (int rc = launch_gemm(P, maps, op, d_gj + g0, g1 - g0, st)) return rc;
         if (prof) CU_TRY(cudaEventRecord(e[1], st));
         {
             const int v8 = P.nt * 8;
@@ -638,7 +653,7 @@ int triples_w_block(int nocc, int nvirt, const double* t2, const double* vvvo, c
                      {k, i, j, 2, ubase + 2 * ub, nullptr, 1, {0, 0, 0}}};
     GemmJob* d_gj = reinterpret_cast<GemmJob*>(ws + P.off_gjobs);
     CU_TRY(cudaMemcpyAsync(d_gj, gj, sizeof gj, cudaMemcpyHostToDevice, st));
-    if (int rc = launch_gemm(P, maps, d_gj, 3, st)) return rc;
+    if (int rc = launch_gemm(P, maps, op, d_gj, 3, st)) return rc;
     if (precision == TRIPLES_FP64)
         assemble_w_kernel<double><<<kNumSM * 4, 256, 0, st>>>((const double*)ubase, nvirt, P.nt, W_out);
     else

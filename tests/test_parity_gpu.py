@@ -273,6 +273,31 @@ def test_zero_inputs_and_scaling_on_gpu():
     assert rel(Es[0], lam * lam * E[0]) <= 1e-12 and abs(Es[2]) == 0.0 and abs(E[2]) == 0.0
 
 
+@pytest.mark.parametrize("lam,mu", [(1.0, 1.0), (3e-9, 2e5), (4e6, 7e-8), (1e-20, 1e12)])
+def test_mixed_path_magnitudes_far_from_one(lam, mu):
+    """The FP16 split scales each tensor class by a power of two (Q13): amplitudes / integrals of any
+    overall magnitude must give the same relative accuracy.  t2 -> lam t2, integrals -> mu g: E4 ~ lam^2 mu^2."""
+    inp = synth.make_inputs(5, 41, 60, seed=6, t1_sigma=0.3)
+    s = synth.TriplesInputs(inp.nocc, inp.nvirt, inp.eps_o, inp.eps_v, inp.t1, inp.t2 * lam, inp.vvvo * mu,
+                            inp.ovoo * mu, inp.ovov * mu)
+    E = gpu_energy(s, prec=tb.MIXED)
+    Eo = oracle.energy_restricted(s.nocc, s.nvirt, *s.arrays())
+    assert rel(E[0], Eo[0]) <= TOL[tb.MIXED] and rel(E[1], Eo[1]) <= TOL[tb.MIXED]
+    assert abs(E[2] - Eo[2]) <= TOL[tb.MIXED] * max(abs(Eo[2]), 1e-3 * abs(Eo[1]))
+
+
+def test_mixed_path_wide_dynamic_range_amplitudes():
+    """Amplitudes spread over 12 orders of magnitude (row-wise factors): elements far below the tensor maximum fall to
+    the split's absolute floor (2^-39 of the maximum), which must not hurt the energy."""
+    inp = synth.make_inputs(5, 41, 60, seed=7, t1_sigma=0.0)
+    f = np.logspace(0, -6, inp.nvirt)
+    t2 = inp.t2 * f[None, None, :, None] * f[None, None, None, :]      # keeps t2[i,j,a,b] = t2[j,i,b,a]
+    s = synth.TriplesInputs(inp.nocc, inp.nvirt, inp.eps_o, inp.eps_v, inp.t1, t2, inp.vvvo, inp.ovoo, inp.ovov)
+    E = gpu_energy(s, prec=tb.MIXED)
+    Eo = oracle.energy_restricted(s.nocc, s.nvirt, *s.arrays())
+    assert rel(E[0], Eo[0]) <= TOL[tb.MIXED]
+
+
 def test_host_entry_point_matches_device_entry_point():
     inp = synth.make_inputs(6, 40, 50, seed=4, t1_sigma=0.1)
     o, v = inp.nocc, inp.nvirt
