@@ -62,8 +62,8 @@ struct GemmF64Cfg {
 
 template <int WM, int WN, int NT, int STAGES>
 __global__ void __launch_bounds__(GemmF64Cfg<WM, WN, NT, STAGES>::THREADS, 1)
-gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict__ jobs, int v, int vp, int o,
-                int mtiles) {
+gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict__ jobs, int njobs, int v, int vp,
+                int o, int mtiles, int ntiles) {
     using C = GemmF64Cfg<WM, WN, NT, STAGES>;
     constexpr int MT = C::MT;
     extern __shared__ uint8_t smem_raw[];
@@ -72,9 +72,10 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
     uint64_t* empty = full + STAGES;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const GemmJob job = jobs[blockIdx.y];
-    const int mt_idx = blockIdx.x % mtiles, nt_idx = blockIdx.x / mtiles;
-    const int m0 = mt_idx * C::BM, n0 = nt_idx * C::BN;
+    // persistent: one CTA per SM walks work items (job, m-tile, n-tile), tiles of a job side by side on the SMs; the
+    // producer runs ahead into the next item while the consumers store the previous one
+    const int per_job = mtiles * ntiles;
+    const long long nitems = (long long)njobs * per_job;
     const int N = v * vp;
     const int nchv = (v + 15) >> 4, ncho = (o + 15) >> 4;
     const int nch = 2 * (nchv + ncho);
@@ -93,10 +94,14 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
         if (lane == 0) {
             tma_prefetch_desc(&maps.t2a); tma_prefetch_desc(&maps.ota); tma_prefetch_desc(&maps.x);
             tma_prefetch_desc(&maps.xt);  tma_prefetch_desc(&maps.t2bq); tma_prefetch_desc(&maps.t2br);
-            const int p = job.p, q = job.q, r = job.r;
-            for (int c = 0; c < nch; ++c) {
-                const int s = c % STAGES;
-                const uint32_t ph = (c / STAGES) & 1;
+            uint32_t it = 0;
+            for (long long w = blockIdx.x; w < nitems; w += gridDim.x) {
+            const int jb = (int)(w / per_job), tile = (int)(w % per_job);
+            const int m0 = (tile % mtiles) * C::BM, n0 = (tile / mtiles) * C::BN;
+            const int p = jobs[jb].p, q = jobs[jb].q, r = jobs[jb].r;
+            for (int c = 0; c < nch; ++c, ++it) {
+                const int s = it % STAGES;
+                const uint32_t ph = (it / STAGES) & 1;
                 mbar_wait(&empty[s], ph ^ 1);
                 uint8_t* sA = smem + s * C::STAGE_BYTES;
                 uint8_t* sB = sA + C::A_BYTES;
@@ -123,6 +128,7 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
                         tma_load_3d(sB + bx * 2048, &maps.t2br, &full[s], n0 + bx * 16, r, kk);
                 }
             }
+            }
         }
         return;
     }
@@ -145,16 +151,20 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
             offB[ntp][up] = (wn * (NT / 2)) * 2048 + t * 128 + (((((nug >> 1) + 2 * ntp) ^ (4 * up + t)) & 7) << 4) +
                             (nug & 1) * 8;
 
+    const uint32_t smem_base = smem_u32(smem);
+    uint32_t it = 0;
+    for (long long w = blockIdx.x; w < nitems; w += gridDim.x) {
+    const int jb = (int)(w / per_job), tile = (int)(w % per_job);
+    const int m0 = (tile % mtiles) * C::BM, n0 = (tile / mtiles) * C::BN;
     double acc[MT][NT][2];
 #pragma unroll
     for (int i = 0; i < MT; ++i)
 #pragma unroll
         for (int j = 0; j < NT; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    const uint32_t smem_base = smem_u32(smem);
-    for (int c = 0; c < nch; ++c) {
-        const int s = c % STAGES;
-        const uint32_t ph = (c / STAGES) & 1;
+    for (int c = 0; c < nch; ++c, ++it) {
+        const int s = it % STAGES;
+        const uint32_t ph = (it / STAGES) & 1;
         int rem;  // valid k left in this segment from the chunk start
         if (c < nchv) rem = v - c * 16;
         else if (c < 2 * nchv) rem = v - (c - nchv) * 16;
@@ -184,8 +194,8 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
 
     // ---------------------------------------------------------------- epilogue: blocked + swizzled store (ulayout.cuh)
     // column n = b*vp + c (c even): the pair (c, c+1) is one 16-byte word of the 8x8x8 block of (row, b, c)
-    double* __restrict__ out = static_cast<double*>(job.out);
-    double* __restrict__ out2 = static_cast<double*>(job.out2);
+    double* __restrict__ out = static_cast<double*>(jobs[jb].out);
+    double* __restrict__ out2 = static_cast<double*>(jobs[jb].out2);
     const int nt = u_tiles(v);
 #pragma unroll
     for (int j = 0; j < NT; ++j) {
@@ -204,6 +214,7 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
             }
         }
     }
+    }   // work items
 }
 
 }  // namespace tb

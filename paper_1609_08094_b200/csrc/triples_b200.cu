@@ -122,8 +122,10 @@ int launch_gemm_f64(const GemmMaps& maps, const GemmJob* jobs, int njobs, const 
         CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
         attr_set = true;
     }
-    dim3 grid(P.mtiles * P.ntiles, njobs);
-    kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(maps, jobs, P.v, P.vp, P.o, P.mtiles);
+    const long long items = (long long)P.mtiles * P.ntiles * njobs;
+    if (items == 0) return TRIPLES_OK;
+    const int grid = (int)std::min<long long>(items, kNumSM);     // persistent: one CTA per SM
+    kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(maps, jobs, njobs, P.v, P.vp, P.o, P.mtiles, P.ntiles);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     return TRIPLES_OK;
