@@ -68,7 +68,7 @@ struct alignas(64) Tf32Maps {
 
 constexpr int TF_BM = 128;            // (b,c) rows per CTA tile = TMEM lanes
 constexpr int TF_BK = 32;             // floats per K chunk (128-byte rows)
-constexpr int TF_THREADS = 512;         // 8 service warps (TMA, MMA, TMEM, 4 converters) + 8 accumulator warps
+constexpr int TF_THREADS = 512;         // 8 service warps (TMA, MMA, 6 converters) + 8 accumulator warps
 constexpr int TF_CONV_WARPS = 6;        // warps 2..7
 constexpr int TF_CHAIN = 2;             // K chunks per TMEM accumulation chain
 constexpr int TF_TMEM_COLS = 512;
@@ -79,8 +79,9 @@ constexpr int TF_MAX_JOBS = 192;        // jobs per launch (3 per triplet, plan.
 constexpr int TF_TAIL_BYTES = 2048 + TF_MAX_JOBS * 48;   // alignment slack + barriers, job table
 
 // npad = N-side rows a CTA stages = bn / 2.  Two shared-memory rings of (128 + npad)-row tiles with 128-byte rows:
-// TF_RAW_STAGES raw tiles (TMA destination, TF32 operand; deep enough to cover the L2/HBM latency) and TF_PK_STAGES
-// packed BF16 tiles (written by the converter warps; the conversion of chunk c+1 overlaps the MMAs of chunk c).
+// TF_RAW_STAGES raw FP32 tiles (TMA destination, read by the converter warps only; deep enough to cover the L2/HBM
+// latency) and TF_PK_STAGES packed FP16 tiles (h | l; written by the converter warps, read by the MMAs; the conversion
+// of later chunks overlaps the MMAs of chunk c).
 constexpr int TF_RAW_STAGES = 3, TF_PK_STAGES = 3;
 __host__ __device__ constexpr int tf32_tile_bytes(int npad) { return (TF_BM + npad) * 128; }
 // the request is always > half an SM's shared memory: exactly one CTA per SM (it owns all 512 TMEM columns)
@@ -111,7 +112,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
     uint8_t* smem_pk = smem + RS * tile_bytes;
     uint8_t* smem_tail = smem_pk + PS * tile_bytes;
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_tail);   // [RS] raw tile landed (per CTA)
-    uint64_t* empty = full + RS;                 // [RS] raw tile consumed by the MMAs
+    uint64_t* empty = full + RS;                 // [RS] raw tile read by this CTA's converter warps
     uint64_t* conv = empty + RS;                 // [PS] packed tile written by both CTAs' converters (leader's is used)
     uint64_t* pkempty = conv + PS;               // [PS] packed tile consumed by the MMAs
     uint64_t* tfull = pkempty + PS;              // accumulator buffer ready for the epilogue
