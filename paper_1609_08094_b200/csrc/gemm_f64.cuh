@@ -42,6 +42,18 @@ struct alignas(64) GemmMaps {
     CUtensorMap t2br;  // t2 as B, rows l at fixed inner index: (n, y, x) box (16, 1, 16)
 };
 
+// Work item w -> (job, tile).  The jobs of a launch are sorted by (q,r) (triples_b200.cu); the gsize jobs of a group
+// share their M-side operand slices XK_r / XKT_q / T2K_q / T2KT_r, so consecutive items are the SAME tile of the
+// group's jobs: the CTAs running side by side then pull identical M-side rows, and the (vv|vo) slices come from HBM
+// once per group instead of once per job (they are far larger than L2: 2 x v^3 x 8 bytes per job).
+__device__ __forceinline__ void grouped_item(const GemmJob* __restrict__ jobs, long long w, int per_job, int& jb, int& rem) {
+    const int any = (int)(w / per_job);                       // some job of the group item w falls in
+    const int gs = jobs[any].gstart, gn = jobs[any].gsize;
+    const long long local = w - (long long)gs * per_job;
+    jb = gs + (int)(local % gn);
+    rem = (int)(local / gn);
+}
+
 __host__ __device__ constexpr int rho_row(int g) { return 2 * (g & 3) + (g >> 2); }                 // MMA row -> tile row
 __host__ __device__ constexpr int nu_col(int g) { return (g & 1) | (((g >> 2) & 1) << 1) | (((g >> 1) & 1) << 3); }
 
@@ -96,7 +108,8 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
             tma_prefetch_desc(&maps.xt);  tma_prefetch_desc(&maps.t2bq); tma_prefetch_desc(&maps.t2br);
             uint32_t it = 0;
             for (long long w = blockIdx.x; w < nitems; w += gridDim.x) {
-            const int jb = (int)(w / per_job), tile = (int)(w % per_job);
+            int jb, tile;
+            grouped_item(jobs, w, per_job, jb, tile);
             const int m0 = (tile % mtiles) * C::BM, n0 = (tile / mtiles) * C::BN;
             const int p = jobs[jb].p, q = jobs[jb].q, r = jobs[jb].r;
             for (int c = 0; c < nch; ++c, ++it) {
@@ -154,7 +167,8 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
     const uint32_t smem_base = smem_u32(smem);
     uint32_t it = 0;
     for (long long w = blockIdx.x; w < nitems; w += gridDim.x) {
-    const int jb = (int)(w / per_job), tile = (int)(w % per_job);
+    int jb, tile;
+    grouped_item(jobs, w, per_job, jb, tile);
     const int m0 = (tile % mtiles) * C::BM, n0 = (tile / mtiles) * C::BN;
     double acc[MT][NT][2];
 #pragma unroll

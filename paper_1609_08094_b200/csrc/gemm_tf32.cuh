@@ -32,7 +32,7 @@
 // a pair walks work items (job, two consecutive m-tiles of 128 (b,c) rows, n-tile of BN a-columns) as ONE
 // 256 x BN MMA tile.  Each CTA stages only its own 128 M-side rows and HALF of the N-side rows (the tensor cores
 // read the other half from the peer's shared memory).  Jobs of a launch are grouped by (q,r) so that the big
-// XK_r / XKT_q slices come from HBM once per group (tf32_item below).
+// XK_r / XKT_q slices come from HBM once per group (grouped_item, gemm_f64.cuh).
 //   warp 0    : TMA producer   (K chunks of 32 words = one 128-byte swizzled row per operand row, ring of 3 raw tiles)
 //   warp 1    : MMA issuer     (one lane of the LEADER CTA; per K chunk 2+2 cross-term MMAs, then 2 main-term MMAs,
 //                               all FP16 K = 16; tcgen05.commit multicasts to both CTAs' barriers)
@@ -87,18 +87,6 @@ __host__ __device__ constexpr int tf32_tile_bytes(int npad) { return (TF_BM + np
 // the request is always > half an SM's shared memory: exactly one CTA per SM (it owns all 512 TMEM columns)
 __host__ __device__ constexpr int tf32_smem_bytes(int npad) {
     return (TF_RAW_STAGES + TF_PK_STAGES) * tf32_tile_bytes(npad) + TF_TAIL_BYTES;
-}
-
-// Work item w -> (job, tile).  The jobs of a launch are sorted by (q,r) (triples_b200.cu); the gsize jobs of a group
-// share their M-side operand slices XK_r / XKT_q / T2K_q / T2KT_r, so consecutive items are the SAME tile of the
-// group's jobs: the CTAs running side by side then pull identical M-side rows, and the (vv|vo) slices come from HBM
-// once per group instead of once per job (they are far larger than L2: 2 x v^3 x 8 bytes per job).
-__device__ __forceinline__ void tf32_item(const GemmJob* __restrict__ jobs, long long w, int per_job, int& jb, int& rem) {
-    const int any = (int)(w / per_job);                       // some job of the group item w falls in
-    const int gs = jobs[any].gstart, gn = jobs[any].gsize;
-    const long long local = w - (long long)gs * per_job;
-    jb = gs + (int)(local % gn);
-    rem = (int)(local / gn);
 }
 
 __global__ void __launch_bounds__(TF_THREADS, 1)
@@ -156,7 +144,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
             uint32_t it = 0;
             for (long long w = cid; w < nitems; w += ncl) {
                 int jb, rem;
-                tf32_item(jobs, w, per_job, jb, rem);
+                grouped_item(jobs, w, per_job, jb, rem);
                 const int m0 = ((rem / ntiles) * cs + rank) * TF_BM;
                 const int an = (rem % ntiles) * bn + rank * npad;   // this CTA's half of the N-side rows
                 const GemmJob job = jobs[jb];
@@ -278,7 +266,7 @@ gemm_tf32_kernel(const __grid_constant__ Tf32Maps maps, const GemmJob* __restric
         uint32_t chain = 0;
         for (long long w = cid; w < nitems; w += ncl) {
             int jb, rem;
-            tf32_item(jobs, w, per_job, jb, rem);
+            grouped_item(jobs, w, per_job, jb, rem);
             const int m0 = ((rem / ntiles) * cs + rank) * TF_BM, a0 = (rem % ntiles) * bn;
             uint64_t acc2[64];          // 128 FP32 running sums as 64 register pairs (packed add.rn.f32x2)
 #pragma unroll
