@@ -212,7 +212,7 @@ int launch_gemm(const Plan& P, const Maps& maps, const Operands& op, const GemmJ
     if (P.prec == TRIPLES_MIXED) return launch_gemm_tf32(maps.tf32, jobs, njobs, P, op.scales, st);
     switch (P.cfg) {
         case CFG_M120_N128: return launch_gemm_f64<3, 4, 4, 4>(maps.f64, jobs, njobs, P, st);
-        case CFG_M80_N192: return launch_gemm_f64<2, 4, 6, 4>(maps.f64, jobs, njobs, P, st);
+        case CFG_M80_N192: return launch_gemm_f64<2, 6, 4, 4>(maps.f64, jobs, njobs, P, st);
         default: return launch_gemm_f64<1, 8, 4, 4>(maps.f64, jobs, njobs, P, st);
     }
 }
