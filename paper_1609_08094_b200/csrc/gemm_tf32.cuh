@@ -33,10 +33,10 @@
 // 256 x BN MMA tile.  Each CTA stages only its own 128 M-side rows and HALF of the N-side rows (the tensor cores
 // read the other half from the peer's shared memory).  Jobs of a launch are grouped by (q,r) so that the big
 // XK_r / XKT_q slices come from HBM once per group (grouped_item, gemm_f64.cuh).
-//   warp 0    : TMA producer   (K chunks of 32 words = one 128-byte swizzled row per operand row, ring of 3 raw tiles)
+//   warp 0    : TMA producer   (K chunks of 32 words = one 128-byte swizzled row per operand row, ring of 4 raw tiles)
 //   warp 1    : MMA issuer     (one lane of the LEADER CTA; per K chunk 2+2 cross-term MMAs, then 2 main-term MMAs,
 //                               all FP16 K = 16; tcgen05.commit multicasts to both CTAs' barriers)
-//   warps 2-7 : converters     (raw tile -> packed tile, ring of 3; warp 2 also allocates TMEM: 512 columns =
+//   warps 2-7 : converters     (raw tile -> packed tile, ring of 2; warp 2 also allocates TMEM: 512 columns =
 //                               two 128 x 256 FP32 buffers in each CTA)
 //   warps 8-15: accumulators   (tcgen05.ld of every finished chain, packed FP32 round-to-nearest adds (FADD2) in
 //                               registers, one 256-bit store per (b,c) row and a-tile of U at the end of the item)
@@ -82,7 +82,7 @@ constexpr int TF_TAIL_BYTES = 2048 + TF_MAX_JOBS * 48;   // alignment slack + ba
 // TF_RAW_STAGES raw FP32 tiles (TMA destination, read by the converter warps only; deep enough to cover the L2/HBM
 // latency) and TF_PK_STAGES packed FP16 tiles (h | l; written by the converter warps, read by the MMAs; the conversion
 // of later chunks overlaps the MMAs of chunk c).
-constexpr int TF_RAW_STAGES = 3, TF_PK_STAGES = 3;
+constexpr int TF_RAW_STAGES = 4, TF_PK_STAGES = 2;
 __host__ __device__ constexpr int tf32_tile_bytes(int npad) { return (TF_BM + npad) * 128; }
 // the request is always > half an SM's shared memory: exactly one CTA per SM (it owns all 512 TMEM columns)
 __host__ __device__ constexpr int tf32_smem_bytes(int npad) {
