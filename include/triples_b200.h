@@ -32,6 +32,8 @@
  *     non-OK status of the calling thread is available from triples_last_error().
  *     There is no CPU fallback: on a device that is not compute capability 10.x the compute
  *     entry points return TRIPLES_EARCH.
+ *   - Device pointers are validated with cudaPointerGetAttributes: a host pointer where a device pointer is
+ *     expected returns TRIPLES_EINVAL (it does not surface as a CUDA fault later).
  *   - precision: TRIPLES_FP64  = contractions in FP64 (DMMA), everything FP64;
  *                TRIPLES_MIXED = the paper's mixed precision (L125, L156): only the W build
  *                (the contractions) in single precision (operands scaled by a power of two and split
@@ -99,6 +101,89 @@ int triples_energy_host(int nocc, int nvirt,
                         double* e_out, double* e_triplet_out);
 
 /*
+ * Triplet-sharded run ("each loop cycle is data independent ... trivially
+ * distributed", L121, L206): the batches (window blocks) of the restricted loop are cut into `nshards` contiguous
+ * ranges of equal contraction-job count (triples_plan_shards); this call computes range `shard` only.
+ * Inputs are replicated.  e_out = this shard's partial (E(T), E[4], E[5]); the caller adds the partials of all
+ * shards in shard order (three doubles per rank -- the only exchange step).  e_triplet_out rows of other shards
+ * are zero.  triples_energy is the case shard = 0, nshards = 1.
+ */
+int triples_energy_sharded(int nocc, int nvirt,
+                           const double* eps_o, const double* eps_v, const double* t1, const double* t2,
+                           const double* vvvo, const double* ovoo, const double* ovov,
+                           int precision, int shard, int nshards,
+                           void* workspace, size_t workspace_bytes, void* cuda_stream,
+                           double* e_out, double* e_triplet_out);
+
+/* Host-side view of that partition: shard_of_triplet (host, T ints or NULL; -1 for i=j=k), jobs_per_shard (host,
+ * nshards long longs or NULL).  Returns the number of batches or -1 on invalid arguments. */
+long long triples_plan_shards(int nocc, int nvirt, int precision, int nshards, int* shard_of_triplet,
+                              long long* jobs_per_shard);
+
+/*
+ * Out-of-core run ("tiles of t2 and ERIs transferred asynchronously, pinned
+ * memory"; L216, L220: sizes "as large as allowed by host memory").  The (vv|vo) integrals stay in HOST memory,
+ * slice-major:   vovv_host[k][a][b][c] = (ab|ck)   (nocc slices of nvirt^3 doubles, pinned for full copy speed);
+ * every other input is device-resident as in triples_energy.  The device keeps a cache of repacked slices X_r
+ * (+ XT_r): as many slots as `workspace_bytes` allows (triples_cache_slots), at least the slices of two
+ * consecutive batches.  A batch is a block of occupied-index windows of width `win` <= 4; a small budget is met
+ * by a narrower window (fewer U buffers, 6 win slices minimum): the call takes the widest window whose minimum
+ * fits, then the largest cache.  Which slice sits in which slot when is planned
+ * on the host for the whole launch order (Belady replacement, triples_plan_slices); the copies of batch b+2 run
+ * on a library-owned copy stream while batch b+1 computes.  Same kernels and the same batches as triples_energy:
+ * per-triplet energies are bitwise identical to the resident run.
+ *   vvvo_absmax : TRIPLES_MIXED only: the largest |(ab|ck)| if the caller knows it (it fixes the power-of-two
+ *                 operand scale); <= 0: the library scans the host tensor once (one extra pass of copies).
+ */
+int triples_energy_streamed(int nocc, int nvirt,
+                            const double* eps_o, const double* eps_v, const double* t1, const double* t2,
+                            const double* vovv_host, const double* ovoo, const double* ovov,
+                            int precision, double vvvo_absmax,
+                            void* workspace, size_t workspace_bytes, void* cuda_stream,
+                            double* e_out, double* e_triplet_out);
+
+/* Workspace bytes of triples_energy_streamed with a slice cache of `nslots` slots (clamped to [minimum, nocc];
+ * nslots <= 0: the minimum) and windows of width <= `win` (win <= 0: the default of the resident run).
+ * 0 on invalid arguments. */
+size_t triples_workspace_bytes_streamed(int nocc, int nvirt, int precision, int nslots, int win);
+
+/*
+ * RI-direct run (Eq. (2.1.3): (pq|rs) = sum_Q B[Q,p,q] B[Q,r,s]).
+ * The vvvo tensor is never materialised: a slice X_r[d,b,c] = sum_Q B[Q,d,b] B[Q,c,r] is rebuilt on the device
+ * by an FP64 DMMA GEMM (M = v^2, N = v, K = naux) whenever a batch needs it and the slice cache does not hold it.
+ *   B : device, [naux][n][n] doubles, n = nocc + nvirt, occupied orbitals first, symmetric in the orbital pair.
+ * ovoo / ovov / t2 are passed as for triples_energy.  Extra work: 2 naux v^3 flop per slice built
+ * (triples_last_profile out[11], out[13]); with a cache of nocc slots every slice is built once.
+ * TRIPLES_MIXED: slices are built in FP64 and split-packed; the operand scale comes from the Cauchy-Schwarz bound
+ * |(ab|ck)| <= |B[:,a,b]| |B[:,c,k]|.
+ */
+int triples_energy_ri(int nocc, int nvirt, int naux,
+                      const double* eps_o, const double* eps_v, const double* t1, const double* t2,
+                      const double* B, const double* ovoo, const double* ovov,
+                      int precision,
+                      void* workspace, size_t workspace_bytes, void* cuda_stream,
+                      double* e_out, double* e_triplet_out);
+
+size_t triples_workspace_bytes_ri(int nocc, int nvirt, int naux, int precision, int nslots, int win);
+
+/* Slice-cache slots a workspace of `workspace_bytes` gives (mode 1 = streamed, 2 = RI; naux: RI only) and, in
+ * *win_out (host or NULL), the window width the run will use; 0 if not even window 1 fits. */
+int triples_cache_slots(int nocc, int nvirt, int naux, int precision, int mode, size_t workspace_bytes, int* win_out);
+
+/*
+ * Host-side plan of the slice cache (pure host arithmetic): for the full restricted loop, a cache of `nslots`
+ * slots and windows of width <= `win` (both clamped as above) in `mode` (1 = streamed: a batch's loads may not
+ * evict what the previous batch uses; 2 = RI), which slice is loaded into which slot before which batch.
+ *   loads_out : host, 3*loads_cap ints or NULL: {batch, r, slot} per load, in order
+ *   jobs_out  : host, 5*jobs_cap ints or NULL: per contraction job in launch order
+ *               {batch, q, r, cache slot of XT_q, cache slot of X_r}
+ *   info_out  : host, 4 ints or NULL: {slots used, window width, batches, jobs}
+ * Returns the number of loads, or -1 on error.
+ */
+long long triples_plan_slices(int nocc, int nvirt, int precision, int mode, int nslots, int win, int* loads_out,
+                              long long loads_cap, int* jobs_out, long long jobs_cap, int* info_out);
+
+/*
  * Per-triplet energies of a caller-chosen list of restricted triplets (the sampled-parity
  * protocol for the configurations whose full oracle run is out of reach).
  *   ntrip, ijk (host, 3*ntrip ints, each 0 <= i <= j <= k < nocc)
@@ -133,9 +218,12 @@ int triples_w_block(int nocc, int nvirt,
  *   out[6] other launches               out[7] contraction flops executed (12v^4+12ov^3 per
  *                                              triplet, coinciding terms of i=j / j=k computed once)
  *   out[8] reduction algorithmic bytes  out[9] triplets executed (i=j=k skipped)
+ *   out[10] per-batch slice work, summed ms (streamed: repack of arrived slices; RI: slice GEMMs + repack)
+ *   out[11] slices loaded / built       out[12] host->device bytes of streamed slices
+ *   out[13] flops of the RI slice GEMMs out[14..15] reserved (0)
  * Returns TRIPLES_EINVAL if no profiled call has happened.
  */
-int triples_last_profile(double* out10);
+int triples_last_profile(double* out16);
 void triples_set_profiling(int on);
 
 /*
@@ -152,6 +240,14 @@ void triples_set_profiling(int on);
  */
 long long triples_plan_batches(int nocc, int nvirt, int precision, int* batch_of_triplet, int* jobs_out,
                                long long* njobs_out);
+
+/*
+ * FP64 tensor-core (mma.sync.m8n8k4.f64, DMMA) peak of the current device in TFLOP/s: a register-resident DMMA
+ * loop on every SM, best of three timed repetitions of `iters` iterations (CUDA events on `cuda_stream`).  This is
+ * the roofline denominator of the FP64 contraction kernel, measured in the process that measures the numerator.
+ * workspace: device, at least 148*256*8 bytes.
+ */
+int triples_probe_fp64_peak(void* workspace, size_t workspace_bytes, void* cuda_stream, int iters, double* tflops_out);
 
 /* Number of CUDA kernels the calling thread's last compute call (triples_energy / _host / _subset / _w_block)
  * launched (repack + contraction + reduction + finalize + total). */

@@ -8,16 +8,25 @@ from .binding import (  # noqa: F401
     FP64,
     MIXED,
     TriplesError,
+    triples_cache_slots,
     triples_energy,
     triples_energy_host,
+    triples_energy_ri,
+    triples_energy_sharded,
+    triples_energy_streamed,
     triples_energy_subset,
     triples_last_launch_count,
     triples_last_profile,
     triples_plan_batches,
+    triples_plan_shards,
+    triples_plan_slices,
+    triples_probe_fp64_peak,
     triples_set_profiling,
     triples_triplet_count,
     triples_triplet_list,
     triples_w_block,
     triples_workspace_bytes,
     triples_workspace_bytes_host,
+    triples_workspace_bytes_ri,
+    triples_workspace_bytes_streamed,
 )

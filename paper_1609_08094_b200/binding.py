@@ -57,6 +57,27 @@ def lib() -> ctypes.CDLL:
             f = getattr(L, name)
             f.argtypes = [ctypes.c_int, ctypes.c_int] + [vp] * 7 + [ctypes.c_int, vp, ctypes.c_size_t, vp, dp, vp]
             f.restype = ctypes.c_int
+        L.triples_energy_sharded.argtypes = ([ctypes.c_int, ctypes.c_int] + [vp] * 7 + [ctypes.c_int] * 3 +
+                                             [vp, ctypes.c_size_t, vp, dp, vp])
+        L.triples_energy_sharded.restype = ctypes.c_int
+        L.triples_energy_streamed.argtypes = ([ctypes.c_int, ctypes.c_int] + [vp] * 7 + [ctypes.c_int, ctypes.c_double] +
+                                              [vp, ctypes.c_size_t, vp, dp, vp])
+        L.triples_energy_streamed.restype = ctypes.c_int
+        L.triples_energy_ri.argtypes = ([ctypes.c_int] * 3 + [vp] * 7 + [ctypes.c_int] +
+                                        [vp, ctypes.c_size_t, vp, dp, vp])
+        L.triples_energy_ri.restype = ctypes.c_int
+        L.triples_workspace_bytes_streamed.argtypes = [ctypes.c_int] * 5
+        L.triples_workspace_bytes_streamed.restype = ctypes.c_size_t
+        L.triples_workspace_bytes_ri.argtypes = [ctypes.c_int] * 6
+        L.triples_workspace_bytes_ri.restype = ctypes.c_size_t
+        L.triples_cache_slots.argtypes = [ctypes.c_int] * 5 + [ctypes.c_size_t, ip]
+        L.triples_cache_slots.restype = ctypes.c_int
+        L.triples_plan_shards.argtypes = [ctypes.c_int] * 4 + [ip, ctypes.POINTER(ctypes.c_longlong)]
+        L.triples_plan_shards.restype = ctypes.c_longlong
+        L.triples_plan_slices.argtypes = [ctypes.c_int] * 6 + [ip, ctypes.c_longlong, ip, ctypes.c_longlong, ip]
+        L.triples_plan_slices.restype = ctypes.c_longlong
+        L.triples_probe_fp64_peak.argtypes = [vp, ctypes.c_size_t, vp, ctypes.c_int, dp]
+        L.triples_probe_fp64_peak.restype = ctypes.c_int
         L.triples_energy_subset.argtypes = ([ctypes.c_int, ctypes.c_int] + [vp] * 7 +
                                             [ctypes.c_int, ctypes.c_int, ip, vp, ctypes.c_size_t, vp, dp])
         L.triples_energy_subset.restype = ctypes.c_int
@@ -72,18 +93,29 @@ def _check(rc: int):
         raise TriplesError(rc, lib().triples_last_error().decode())
 
 
-def _dev_ptr(t, name):
+def _dev_ptr(t, name, numel=None):
     import torch
 
     if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
         raise TypeError(f"{name}: expected a contiguous float64 CUDA tensor")
+    if t.device.index != torch.cuda.current_device():
+        raise ValueError(f"{name}: lives on {t.device}, the current device is cuda:{torch.cuda.current_device()}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{name}: {t.numel()} elements, expected {numel} (the C side cannot see sizes)")
     return ctypes.c_void_p(t.data_ptr())
 
 
-def _host_ptr(a, name):
+def _host_ptr(a, name, numel=None):
     if not isinstance(a, np.ndarray) or a.dtype != np.float64 or not a.flags.c_contiguous:
         raise TypeError(f"{name}: expected a C-contiguous float64 numpy array")
+    if numel is not None and a.size != numel:
+        raise ValueError(f"{name}: {a.size} elements, expected {numel} (the C side cannot see sizes)")
     return ctypes.c_void_p(a.ctypes.data)
+
+
+def _sizes(o, v):
+    """Element counts of (eps_o, eps_v, t1, t2, vvvo, ovoo, ovov) for the layouts of include/triples_b200.h."""
+    return (o, v, o * v, o * o * v * v, v * v * v * o, o * v * o * o, o * v * o * v)
 
 
 def _stream_ptr(stream):
@@ -98,6 +130,9 @@ def _ws(workspace):
 
     if not isinstance(workspace, torch.Tensor) or not workspace.is_cuda or workspace.dtype != torch.uint8:
         raise TypeError("workspace: expected a torch.uint8 CUDA tensor")
+    if workspace.device.index != torch.cuda.current_device():
+        raise ValueError(f"workspace: lives on {workspace.device}, the current device is "
+                         f"cuda:{torch.cuda.current_device()}")
     return ctypes.c_void_p(workspace.data_ptr()), ctypes.c_size_t(workspace.numel())
 
 
@@ -132,10 +167,11 @@ def triples_set_profiling(on: bool) -> None:
 
 
 def triples_last_profile() -> dict:
-    out = (ctypes.c_double * 10)()
+    out = (ctypes.c_double * 16)()
     _check(lib().triples_last_profile(out))
     keys = ("prepare_ms", "contraction_ms", "contraction_launches", "reduction_ms", "reduction_launches",
-            "other_ms", "other_launches", "contraction_flops", "reduction_bytes", "triplets")
+            "other_ms", "other_launches", "contraction_flops", "reduction_bytes", "triplets",
+            "slices_ms", "slices_loaded", "h2d_bytes", "ri_flops")
     return dict(zip(keys, [float(x) for x in out]))
 
 
@@ -153,36 +189,135 @@ def triples_plan_batches(nocc: int, nvirt: int, precision: int):
     return int(nb), bot, jobs[: nj.value].copy()
 
 
+def triples_plan_shards(nocc: int, nvirt: int, precision: int, nshards: int):
+    """(number of batches, shard_of_triplet[T] (-1 for i=j=k), jobs_per_shard[nshards])."""
+    T = triples_triplet_count(nocc)
+    sot = np.empty(max(T, 0), dtype=np.int32)
+    jps = np.zeros(max(nshards, 1), dtype=np.int64)
+    nb = lib().triples_plan_shards(nocc, nvirt, precision, nshards, sot.ctypes.data_as(ctypes.POINTER(ctypes.c_int)),
+                                   jps.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong)))
+    if nb < 0:
+        raise TriplesError(1, lib().triples_last_error().decode())
+    return int(nb), sot, jps
+
+
+def triples_plan_slices(nocc: int, nvirt: int, precision: int, mode: int, nslots: int = 0, win: int = 0):
+    """(loads[n, 3] = {batch, r, slot}, jobs[njobs, 5] = {batch, q, r, slot of XT_q, slot of X_r},
+    info = {"nslots", "win", "batches", "jobs"}) of a streamed (mode 1) / RI (mode 2) run."""
+    T = triples_triplet_count(nocc)
+    cap = 12 * max(T, 1)
+    loads = np.empty((cap, 3), dtype=np.int32)
+    jobs = np.empty((3 * max(T, 1), 5), dtype=np.int32)
+    info = np.zeros(4, dtype=np.int32)
+    ip = ctypes.POINTER(ctypes.c_int)
+    n = lib().triples_plan_slices(nocc, nvirt, precision, mode, nslots, win, loads.ctypes.data_as(ip), cap,
+                                  jobs.ctypes.data_as(ip), jobs.shape[0], info.ctypes.data_as(ip))
+    if n < 0:
+        raise TriplesError(1, lib().triples_last_error().decode())
+    return loads[:n].copy(), jobs[: info[3]].copy(), dict(zip(("nslots", "win", "batches", "jobs"), map(int, info)))
+
+
+def triples_workspace_bytes_streamed(nocc: int, nvirt: int, precision: int, nslots: int = 0, win: int = 0) -> int:
+    return int(lib().triples_workspace_bytes_streamed(nocc, nvirt, precision, nslots, win))
+
+
+def triples_workspace_bytes_ri(nocc: int, nvirt: int, naux: int, precision: int, nslots: int = 0, win: int = 0) -> int:
+    return int(lib().triples_workspace_bytes_ri(nocc, nvirt, naux, precision, nslots, win))
+
+
+def triples_cache_slots(nocc: int, nvirt: int, naux: int, precision: int, mode: int, workspace_bytes: int):
+    """(cache slots, window width) a streamed (mode 1) / RI (mode 2) run gets from a workspace of that size."""
+    win = ctypes.c_int(0)
+    n = int(lib().triples_cache_slots(nocc, nvirt, naux, precision, mode, workspace_bytes, ctypes.byref(win)))
+    return n, int(win.value)
+
+
 def triples_last_launch_count() -> int:
     return int(lib().triples_last_launch_count())
+
+
+def triples_probe_fp64_peak(workspace, stream=None, iters: int = 20000) -> float:
+    """Measured FP64 tensor-core (DMMA) peak of the current device in TFLOP/s."""
+    wp, wn = _ws(workspace)
+    out = ctypes.c_double(0.0)
+    _check(lib().triples_probe_fp64_peak(wp, wn, _stream_ptr(stream), iters, ctypes.byref(out)))
+    return float(out.value)
+
+
+def _e_triplet(e_triplet_out, nocc, host=False):
+    if e_triplet_out is None:
+        return ctypes.c_void_p(None)
+    n = 3 * triples_triplet_count(nocc)
+    return _host_ptr(e_triplet_out, "e_triplet_out", n) if host else _dev_ptr(e_triplet_out, "e_triplet_out", n)
 
 
 def triples_energy(nocc, nvirt, eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, precision, workspace, stream=None,
                    e_triplet_out=None):
     """Device-resident inputs (torch float64 CUDA tensors).  Returns (E(T), E[4], E[5])."""
-    ptrs = [_dev_ptr(t, n) for t, n in zip((eps_o, eps_v, t1, t2, vvvo, ovoo, ovov), _NAMES)]
+    ptrs = [_dev_ptr(t, n, k) for t, n, k in zip((eps_o, eps_v, t1, t2, vvvo, ovoo, ovov), _NAMES, _sizes(nocc, nvirt))]
     wp, wn = _ws(workspace)
     e_out = (ctypes.c_double * 3)()
-    et = ctypes.c_void_p(None) if e_triplet_out is None else _dev_ptr(e_triplet_out, "e_triplet_out")
-    _check(lib().triples_energy(nocc, nvirt, *ptrs, precision, wp, wn, _stream_ptr(stream), e_out, et))
+    _check(lib().triples_energy(nocc, nvirt, *ptrs, precision, wp, wn, _stream_ptr(stream), e_out,
+                                _e_triplet(e_triplet_out, nocc)))
+    return float(e_out[0]), float(e_out[1]), float(e_out[2])
+
+
+def triples_energy_sharded(nocc, nvirt, eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, precision, shard, nshards, workspace,
+                           stream=None, e_triplet_out=None):
+    """This shard's partial (E(T), E[4], E[5]); the caller adds the partials in shard order."""
+    ptrs = [_dev_ptr(t, n, k) for t, n, k in zip((eps_o, eps_v, t1, t2, vvvo, ovoo, ovov), _NAMES, _sizes(nocc, nvirt))]
+    wp, wn = _ws(workspace)
+    e_out = (ctypes.c_double * 3)()
+    _check(lib().triples_energy_sharded(nocc, nvirt, *ptrs, precision, shard, nshards, wp, wn, _stream_ptr(stream),
+                                        e_out, _e_triplet(e_triplet_out, nocc)))
     return float(e_out[0]), float(e_out[1]), float(e_out[2])
 
 
 def triples_energy_host(nocc, nvirt, eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, precision, workspace, stream=None,
                         e_triplet_out=None):
     """Host inputs (numpy float64); host<->device copies happen inside the call."""
-    ptrs = [_host_ptr(a, n) for a, n in zip((eps_o, eps_v, t1, t2, vvvo, ovoo, ovov), _NAMES)]
+    ptrs = [_host_ptr(a, n, k) for a, n, k in zip((eps_o, eps_v, t1, t2, vvvo, ovoo, ovov), _NAMES, _sizes(nocc, nvirt))]
     wp, wn = _ws(workspace)
     e_out = (ctypes.c_double * 3)()
-    et = ctypes.c_void_p(None) if e_triplet_out is None else _host_ptr(e_triplet_out, "e_triplet_out")
-    _check(lib().triples_energy_host(nocc, nvirt, *ptrs, precision, wp, wn, _stream_ptr(stream), e_out, et))
+    _check(lib().triples_energy_host(nocc, nvirt, *ptrs, precision, wp, wn, _stream_ptr(stream), e_out,
+                                     _e_triplet(e_triplet_out, nocc, host=True)))
+    return float(e_out[0]), float(e_out[1]), float(e_out[2])
+
+
+def triples_energy_streamed(nocc, nvirt, eps_o, eps_v, t1, t2, vovv_host, ovoo, ovov, precision, workspace, stream=None,
+                            e_triplet_out=None, vvvo_absmax=0.0):
+    """Out-of-core run: vovv_host[k,a,b,c] = (ab|ck) is a HOST array (numpy, ideally pinned); the rest on the device."""
+    o, v = nocc, nvirt
+    sz = _sizes(o, v)
+    ptrs = [_dev_ptr(t, n, k) for t, n, k in zip((eps_o, eps_v, t1, t2), _NAMES[:4], sz[:4])]
+    ptrs.append(_host_ptr(vovv_host, "vovv_host", sz[4]))
+    ptrs += [_dev_ptr(ovoo, "ovoo", sz[5]), _dev_ptr(ovov, "ovov", sz[6])]
+    wp, wn = _ws(workspace)
+    e_out = (ctypes.c_double * 3)()
+    _check(lib().triples_energy_streamed(o, v, *ptrs, precision, float(vvvo_absmax), wp, wn, _stream_ptr(stream), e_out,
+                                         _e_triplet(e_triplet_out, nocc)))
+    return float(e_out[0]), float(e_out[1]), float(e_out[2])
+
+
+def triples_energy_ri(nocc, nvirt, naux, eps_o, eps_v, t1, t2, B, ovoo, ovov, precision, workspace, stream=None,
+                      e_triplet_out=None):
+    """RI-direct run: B[Q,p,q] (device, [naux, n, n], n = nocc + nvirt) instead of the vvvo tensor."""
+    o, v = nocc, nvirt
+    sz = _sizes(o, v)
+    ptrs = [_dev_ptr(t, n, k) for t, n, k in zip((eps_o, eps_v, t1, t2), _NAMES[:4], sz[:4])]
+    ptrs.append(_dev_ptr(B, "B", naux * (o + v) * (o + v)))
+    ptrs += [_dev_ptr(ovoo, "ovoo", sz[5]), _dev_ptr(ovov, "ovov", sz[6])]
+    wp, wn = _ws(workspace)
+    e_out = (ctypes.c_double * 3)()
+    _check(lib().triples_energy_ri(o, v, naux, *ptrs, precision, wp, wn, _stream_ptr(stream), e_out,
+                                   _e_triplet(e_triplet_out, nocc)))
     return float(e_out[0]), float(e_out[1]), float(e_out[2])
 
 
 def triples_energy_subset(nocc, nvirt, eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, precision, triplets, workspace,
                           stream=None) -> np.ndarray:
     """Weighted per-triplet energies [n,3] for a list of restricted triplets (device inputs)."""
-    ptrs = [_dev_ptr(t, n) for t, n in zip((eps_o, eps_v, t1, t2, vvvo, ovoo, ovov), _NAMES)]
+    ptrs = [_dev_ptr(t, n, k) for t, n, k in zip((eps_o, eps_v, t1, t2, vvvo, ovoo, ovov), _NAMES, _sizes(nocc, nvirt))]
     wp, wn = _ws(workspace)
     trip = np.ascontiguousarray(np.asarray(triplets, dtype=np.int32).reshape(-1, 3))
     out = np.zeros((trip.shape[0], 3), dtype=np.float64)
@@ -194,8 +329,9 @@ def triples_energy_subset(nocc, nvirt, eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, p
 
 def triples_w_block(nocc, nvirt, t2, vvvo, ovoo, precision, i, j, k, workspace, W_out, stream=None):
     """W_ijk^abc of Eq. (2.2.2)-(2.2.3) into W_out (float64 CUDA tensor [v,v,v])."""
-    ptrs = [_dev_ptr(t, n) for t, n in zip((t2, vvvo, ovoo), ("t2", "vvvo", "ovoo"))]
+    sz = _sizes(nocc, nvirt)
+    ptrs = [_dev_ptr(t, n, k_) for t, n, k_ in zip((t2, vvvo, ovoo), ("t2", "vvvo", "ovoo"), (sz[3], sz[4], sz[5]))]
     wp, wn = _ws(workspace)
     _check(lib().triples_w_block(nocc, nvirt, *ptrs, precision, i, j, k, wp, wn, _stream_ptr(stream),
-                                 _dev_ptr(W_out, "W_out")))
+                                 _dev_ptr(W_out, "W_out", nvirt ** 3)))
     return W_out

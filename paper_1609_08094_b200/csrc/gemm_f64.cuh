@@ -29,15 +29,16 @@ struct GemmJob {
     void* out;   // G(p,q,r)[a][b][c] in the blocked layout of ulayout.cuh: slot base + u * UBLK
     void* out2;  // second destination (or null): a triplet with i=j or j=k uses the same G twice
     int gsize;   // i.e. the same X_r / XT_q operand slices: walked tile by tile together
-    int pad[3];
+    int xr, xq;  // slots of the slice cache that hold X_r and XT_q (resident run: xr = r, xq = q)
+    int pad;
 };
 static_assert(sizeof(GemmJob) == 48, "plan.h sizes the job table with 48 bytes per job");
 
 struct alignas(64) GemmMaps {
     CUtensorMap t2a;   // t2 as A: (d, a, pq)          box (16, BM, 1)
     CUtensorMap ota;   // -ovoo as A: (l, a, r*o+p)    box (16, BM, 1)
-    CUtensorMap x;     // X:  (n, d, r)                box (16, 16, 1)
-    CUtensorMap xt;    // XT: (n, d, r)                box (16, 16, 1)
+    CUtensorMap x;     // X:  (n, d, slot)             box (16, 16, 1)
+    CUtensorMap xt;    // XT: (n, d, slot)             box (16, 16, 1)
     CUtensorMap t2bq;  // t2 as B, rows l at fixed outer index: (n, y, x) box (16, 16, 1)
     CUtensorMap t2br;  // t2 as B, rows l at fixed inner index: (n, y, x) box (16, 1, 16)
 };
@@ -70,6 +71,53 @@ struct GemmF64Cfg {
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8 + 1024;  // + barriers + align slack
     static_assert(NT % 2 == 0, "BN must be a multiple of 16 per warp");
     static_assert(A_BYTES % 1024 == 0 && B_BYTES % 1024 == 0, "swizzle atoms are 1 KiB");
+};
+
+// Fragment addressing and the per-chunk DMMA loop of one compute warp (shared by the contraction kernel below and the
+// RI slice builder of ri_slices.cuh).  acc[i][j] = 8x8 accumulator tile (i: 5 row tiles, j: NT column tiles).
+template <int WM, int WN, int NT>
+struct DmmaWarp {
+    static constexpr int MT = 5;
+    uint32_t offA[4], offB[2][2];
+    int rg, t, wm, wn;
+    __device__ __forceinline__ void init(int warp, int lane) {
+        const int g = lane >> 2;
+        t = lane & 3;
+        wm = warp % WM; wn = warp / WM;
+        rg = rho_row(g);
+        const int nug = nu_col(g);
+        // A element (row m, k): byte = m*128 + (((k>>1) ^ (m&7)) << 4) + (k&1)*8, with k = 4u + t
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            offA[u] = (wm * MT * 8 + rg) * 128 + ((((2 * u + (t >> 1)) ^ rg) & 7) << 4) + (t & 1) * 8;
+        // B element (k, n): box n>>4, byte = k*128 + ((((n&15)>>1) ^ (k&7)) << 4) + (n&1)*8, n&15 = nu(g) + 4*(nt&1)
+#pragma unroll
+        for (int ntp = 0; ntp < 2; ++ntp)
+#pragma unroll
+            for (int up = 0; up < 2; ++up)
+                offB[ntp][up] = (wn * (NT / 2)) * 2048 + t * 128 + (((((nug >> 1) + 2 * ntp) ^ (4 * up + t)) & 7) << 4) +
+                                (nug & 1) * 8;
+    }
+    // one staged K chunk of 16: nu = number of k4 steps that carry data
+    __device__ __forceinline__ void chunk(double (&acc)[MT][NT][2], uint32_t sA, uint32_t sB, int nu) const {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (u < nu) {
+                double a[MT], b[NT];
+#pragma unroll
+                for (int i = 0; i < MT; ++i) a[i] = lds_f64(sA + offA[u] + i * 8 * 128);
+#pragma unroll
+                for (int j = 0; j < NT; ++j) b[j] = lds_f64(sB + offB[j & 1][u & 1] + (j >> 1) * 2048 + u * 512);
+#pragma unroll
+                for (int i = 0; i < MT; ++i)
+#pragma unroll
+                    for (int j = 0; j < NT; ++j) dmma_884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+            }
+        }
+    }
+    // output coordinates of acc[i][j][0..1]: row (relative to the tile), column pair (col, col + 1)
+    __device__ __forceinline__ int row(int i) const { return wm * MT * 8 + i * 8 + rg; }
+    __device__ __forceinline__ int col(int j) const { return (wn * (NT / 2) + (j >> 1)) * 16 + (j & 1) * 4 + nu_col(2 * t); }
 };
 
 template <int WM, int WN, int NT, int STAGES>
@@ -111,7 +159,7 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
             int jb, tile;
             grouped_item(jobs, w, per_job, jb, tile);
             const int m0 = (tile % mtiles) * C::BM, n0 = (tile / mtiles) * C::BN;
-            const int p = jobs[jb].p, q = jobs[jb].q, r = jobs[jb].r;
+            const int p = jobs[jb].p, q = jobs[jb].q, r = jobs[jb].r, xr = jobs[jb].xr, xq = jobs[jb].xq;
             for (int c = 0; c < nch; ++c, ++it) {
                 const int s = it % STAGES;
                 const uint32_t ph = (it / STAGES) & 1;
@@ -123,12 +171,12 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
                     const int kk = c * 16;
                     tma_load_3d(sA, &maps.t2a, &full[s], kk, m0, p * o + q);
                     for (int bx = 0; bx < C::BN / 16; ++bx)
-                        tma_load_3d(sB + bx * 2048, &maps.x, &full[s], n0 + bx * 16, kk, r);
+                        tma_load_3d(sB + bx * 2048, &maps.x, &full[s], n0 + bx * 16, kk, xr);
                 } else if (c < 2 * nchv) {                        // sum_d t2[p,r,a,d] XT_q[d,n]
                     const int kk = (c - nchv) * 16;
                     tma_load_3d(sA, &maps.t2a, &full[s], kk, m0, p * o + r);
                     for (int bx = 0; bx < C::BN / 16; ++bx)
-                        tma_load_3d(sB + bx * 2048, &maps.xt, &full[s], n0 + bx * 16, kk, q);
+                        tma_load_3d(sB + bx * 2048, &maps.xt, &full[s], n0 + bx * 16, kk, xq);
                 } else if (c < 2 * nchv + ncho) {                 // -sum_l O_pr[a,l] t2[q,l,n]
                     const int kk = (c - 2 * nchv) * 16;
                     tma_load_3d(sA, &maps.ota, &full[s], kk, m0, r * o + p);
@@ -147,22 +195,8 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
     }
 
     // ---------------------------------------------------------------- DMMA consumers
-    const int g = lane >> 2, t = lane & 3;
-    const int wm = warp % WM, wn = warp / WM;
-    const int rg = rho_row(g), nug = nu_col(g);
-    // A element (row m, k): byte = m*128 + (((k>>1) ^ (m&7)) << 4) + (k&1)*8, with k = 4u + t
-    uint32_t offA[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u)
-        offA[u] = (wm * MT * 8 + rg) * 128 + ((((2 * u + (t >> 1)) ^ rg) & 7) << 4) + (t & 1) * 8;
-    // B element (k, n): box n>>4, byte = k*128 + ((((n&15)>>1) ^ (k&7)) << 4) + (n&1)*8, n&15 = nu(g) + 4*(nt&1)
-    uint32_t offB[2][2];
-#pragma unroll
-    for (int ntp = 0; ntp < 2; ++ntp)
-#pragma unroll
-        for (int up = 0; up < 2; ++up)
-            offB[ntp][up] = (wn * (NT / 2)) * 2048 + t * 128 + (((((nug >> 1) + 2 * ntp) ^ (4 * up + t)) & 7) << 4) +
-                            (nug & 1) * 8;
+    DmmaWarp<WM, WN, NT> dw;
+    dw.init(warp, lane);
 
     const uint32_t smem_base = smem_u32(smem);
     uint32_t it = 0;
@@ -188,20 +222,7 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
         mbar_wait(&full[s], ph);
         const uint32_t sA = smem_base + s * C::STAGE_BYTES;
         const uint32_t sB = sA + C::A_BYTES;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            if (u < nu) {
-                double a[MT], b[NT];
-#pragma unroll
-                for (int i = 0; i < MT; ++i) a[i] = lds_f64(sA + offA[u] + i * 8 * 128);
-#pragma unroll
-                for (int j = 0; j < NT; ++j) b[j] = lds_f64(sB + offB[j & 1][u & 1] + (j >> 1) * 2048 + u * 512);
-#pragma unroll
-                for (int i = 0; i < MT; ++i)
-#pragma unroll
-                    for (int j = 0; j < NT; ++j) dmma_884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-            }
-        }
+        dw.chunk(acc, sA, sB, nu);
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[s]);
     }
@@ -213,13 +234,13 @@ gemm_f64_kernel(const __grid_constant__ GemmMaps maps, const GemmJob* __restrict
     const int nt = u_tiles(v);
 #pragma unroll
     for (int j = 0; j < NT; ++j) {
-        const int col = n0 + (wn * (NT / 2) + (j >> 1)) * 16 + (j & 1) * 4 + nu_col(2 * t);
+        const int col = n0 + dw.col(j);
         const int bb = col / vp, cc = col - bb * vp;
         if (col < N && cc < v) {
             const size_t cb = ((size_t)(bb >> 3) * nt + (cc >> 3)) * UCHUNK;
 #pragma unroll
             for (int i = 0; i < MT; ++i) {
-                const int row = m0 + wm * MT * 8 + i * 8 + rg;
+                const int row = m0 + dw.row(i);
                 if (row < v) {
                     const size_t off = (size_t)(row >> 3) * nt * nt * UCHUNK + cb + u_swz<8>(row & 7, bb & 7, cc & 7);
                     *reinterpret_cast<double2*>(out + off) = make_double2(acc[i][j][0], acc[i][j][1]);

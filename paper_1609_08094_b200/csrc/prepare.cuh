@@ -4,8 +4,11 @@
 //   XT[r][d][b][c] = X[r][d][c][b]
 //   Ot[r][p][a][l] = -ovoo[p][a][l][r] = -(pa|lr)      (l-pitch op = o rounded up to even, pad zeroed)
 //   T2[p][q][a][d] = t2[p][q][a][d]                    (d-pitch vp, pad zeroed)
-// TO is the operand type of the contraction path (double; float = the mixed path's biased FP32 words).
+// TO is the operand type of the FP64 contraction path (double).  The mixed path's operands are written pre-split
+// (FP16 h | l rows, second half of this file).
 #pragma once
+#include <cuda_fp16.h>
+
 #include <cstdint>
 
 namespace tb {
@@ -39,16 +42,10 @@ __global__ void scales_kernel(const unsigned int* __restrict__ maxbits, float* _
     scales[2] = ldexpf(1.0f, -(s[0] + s[1]));
 }
 
-// operand element of the contraction path: the double itself (FP64), or the mixed path's scaled FP32 value
-template <typename TO> __device__ __forceinline__ TO operand_word(double x, double scale);
-template <> __device__ __forceinline__ double operand_word<double>(double x, double) { return x; }
-template <> __device__ __forceinline__ float operand_word<float>(double x, double scale) { return (float)(x * scale); }
-
 // vvvo viewed as [R = v^3][o]: each CTA moves RB consecutive rows (one contiguous span) through smem.
 template <typename TO>
 __global__ void __launch_bounds__(256)
 pack_x_kernel(const double* __restrict__ vvvo, int v, int vp, int o, int RB, TO* __restrict__ X) {
-    const double scale = 1.0;   // FP64 path only
     extern __shared__ double tile[];   // [RB][o+1]
     const size_t R = (size_t)v * v * v;
     const size_t R0 = (size_t)blockIdx.x * RB;
@@ -65,7 +62,7 @@ pack_x_kernel(const double* __restrict__ vvvo, int v, int vp, int o, int RB, TO*
         const size_t Rg = R0 + rr;
         const size_t db = Rg / v;
         const int c = (int)(Rg % v);
-        X[(size_t)k * plane + db * vp + c] = operand_word<TO>(tile[rr * op1 + k], scale);
+        X[(size_t)k * plane + db * vp + c] = (TO)tile[rr * op1 + k];
     }
 }
 
@@ -86,9 +83,7 @@ transpose_planes_kernel(const TO* __restrict__ X, int v, int vp, TO* __restrict_
 
 // Ot[r][p][a][l] = -ovoo[p][a][l][r]
 template <typename TO>
-__global__ void pack_ot_kernel(const double* __restrict__ ovoo, int v, int o, int op, TO* __restrict__ Ot,
-                               const float* __restrict__ scale_ptr) {
-    const double scale = scale_ptr ? (double)*scale_ptr : 1.0;
+__global__ void pack_ot_kernel(const double* __restrict__ ovoo, int v, int o, int op, TO* __restrict__ Ot) {
     const size_t n = (size_t)o * o * v * o;
     for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         const int l = (int)(e % o);
@@ -96,87 +91,133 @@ __global__ void pack_ot_kernel(const double* __restrict__ ovoo, int v, int o, in
         const int p = (int)((e / ((size_t)o * v)) % o);
         const int r = (int)(e / ((size_t)o * v * o));
         const double x = -ovoo[(((size_t)p * v + a) * o + l) * o + r];
-        Ot[(((size_t)r * o + p) * v + a) * op + l] = operand_word<TO>(x, scale);
+        Ot[(((size_t)r * o + p) * v + a) * op + l] = (TO)x;
     }
 }
 
 // T2[p][q][a][d] (d-pitch vp) = t2[p][q][a][d]
 template <typename TO>
-__global__ void pack_t2_kernel(const double* __restrict__ t2, size_t rows, int v, int vp, TO* __restrict__ T2,
-                               const float* __restrict__ scale_ptr) {
-    const double scale = scale_ptr ? (double)*scale_ptr : 1.0;
+__global__ void pack_t2_kernel(const double* __restrict__ t2, size_t rows, int v, int vp, TO* __restrict__ T2) {
     const size_t n = rows * v;
     for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         const size_t row = e / v;
         const int d = (int)(e % v);
-        T2[row * vp + d] = operand_word<TO>(t2[e], scale);
+        T2[row * vp + d] = (TO)t2[e];
     }
 }
 
 // ------------------------------------------------------------------------------------------------ mixed path
-// K-major operands of gemm_tf32.cuh, 4 bytes per element (scaled FP32, see scales_kernel):
-//   XK  [r][b][c][d] = vvvo[d][b][c][r] = (db|cr)      (c: vp rows per b, d-pitch vk = v rounded up to 4)
-//   XKT [r][b][c][d] = XK[r][c][b][d]
-//   T2K [q][b][c][l] = t2[q][l][b][c]                  (l-pitch ok = o rounded up to 4)
+// K-major operands of gemm_f16split.cuh, written SPLIT (Q13): with xs = (float)(x * 2^s) the scaled value,
+// h = RN_fp16(xs), l = RN_fp16(xs - h).  Per operand row and 32-wide K chunk one 128-byte row of 32 words:
+// words 0..15 = the 32 FP16 of h, words 16..31 = the 32 FP16 of l (element k in the low half of word k/2 for even k).
+// K pitches vk / ok = v / o rounded up to 32; K elements beyond v / o are written as zeros.
+//   XK  [s][b][c][d] = (db|cr) of the slice r held in slot s   (c: vp rows per b)
+//   XKT [s][b][c][d] = XK[s][c][b][d]
+//   T2K [q][b][c][l] = t2[q][l][b][c]
 //   T2KT[r][b][c][l] = t2[l][r][b][c] = t2[r][l][c][b]
-//   T2A = pack_t2_kernel with pitch vk, OtA = pack_ot_kernel with pitch ok.
-// Pads are zeroed by the caller (cudaMemsetAsync) when any exists.
+//   T2A [p][q][a][d] = t2[p][q][a][d],  OtA[r][p][a][l] = -ovoo[p][a][l][r]
+// Rows c = v (odd v only) are zeroed by the caller (cudaMemsetAsync).
 
-// vvvo viewed as [d][s = (b,c,r) flat, v*v*o]: one CTA moves a (32 d) x (PKX_SPAN s) brick through smem and writes
-// rows of 32 consecutive d (128 bytes).
+// The 32 lanes of a warp hold 32 consecutive K elements (lane = k within the chunk) and write the chunk's packed row.
+__device__ __forceinline__ void pack_split_store(uint32_t* __restrict__ row, float xs, int lane) {
+    const __half h = __float2half_rn(xs);
+    const __half l = __float2half_rn(xs - __half2float(h));
+    const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
+    const bool odd = (lane & 1) != 0;            // even lane 2j assembles word j (h pair), odd lane 2j+1 word 16+j (l pair)
+    const uint32_t mine = odd ? lb : hb;
+    const uint32_t got = __shfl_xor_sync(0xffffffffu, odd ? hb : lb, 1);
+    row[(lane >> 1) + (odd ? 16 : 0)] = odd ? (got | (mine << 16)) : (mine | (got << 16));
+}
+
+// Source viewed as [d][s], s = bc * ro + r (resident vvvo: ro = o, the slice of r goes to slot r) or s = bc
+// (one streamed slice (ab|c r): ro = 1, slot0 = its slot).  One CTA moves a (32 d) x (PKX_SPAN s) brick through
+// shared memory and writes whole 128-byte packed rows; blockIdx.y = K chunk.
 constexpr int PKX_SPAN = 256;
 constexpr int PKX_PITCH = PKX_SPAN + 1;
 constexpr int PKX_SMEM = 32 * PKX_PITCH * 8;
 __global__ void __launch_bounds__(256)
-pack_xk_kernel(const double* __restrict__ vvvo, int v, int vp, int vk, int o, float* __restrict__ XK,
-               float* __restrict__ XKT, const float* __restrict__ scale_ptr) {
+pack_xk_kernel(const double* __restrict__ src, int v, int vp, int vk, int ro, int slot0, uint32_t* __restrict__ XK,
+               uint32_t* __restrict__ XKT, const float* __restrict__ scale_ptr) {
     const double scale = (double)*scale_ptr;
     extern __shared__ double tile[];                 // [32][PKX_PITCH]
     const int d0 = blockIdx.y * 32;
-    const size_t S = (size_t)v * v * o;
+    const size_t S = (size_t)v * v * ro;
     const size_t s0 = (size_t)blockIdx.x * PKX_SPAN;
     const int cnt = (int)min((size_t)PKX_SPAN, S - s0);
     for (int e = threadIdx.x; e < 32 * cnt; e += 256) {
         const int dd = e / cnt, s = e % cnt;
-        if (d0 + dd < v) tile[dd * PKX_PITCH + s] = vvvo[(size_t)(d0 + dd) * S + s0 + s];
+        tile[dd * PKX_PITCH + s] = d0 + dd < v ? src[(size_t)(d0 + dd) * S + s0 + s] : 0.0;
     }
     __syncthreads();
-    const size_t plane = (size_t)v * vp * vk;        // one r-slice
-    for (int e = threadIdx.x; e < 32 * cnt; e += 256) {
-        const int dd = e & 31, s = e >> 5;
-        if (d0 + dd >= v) continue;
+    const size_t plane = (size_t)v * vp * vk;        // words of one slot
+    const int lane = threadIdx.x & 31;
+    for (int e = threadIdx.x; e < 32 * cnt; e += 256) {      // a warp = the 32 d of one s
+        const int s = e >> 5;
         const size_t sg = s0 + s;
-        const int r = (int)(sg % o);
-        const size_t bc = sg / o;
+        const int r = (int)(sg % ro);
+        const size_t bc = sg / ro;
         const int b = (int)(bc / v), c = (int)(bc % v);
-        const double x = tile[dd * PKX_PITCH + s];
-        const float wd = (float)(x * scale);
-        XK[(size_t)r * plane + ((size_t)b * vp + c) * vk + d0 + dd] = wd;
-        XKT[(size_t)r * plane + ((size_t)c * vp + b) * vk + d0 + dd] = wd;
+        const float xs = (float)(tile[lane * PKX_PITCH + s] * scale);
+        const size_t base = (size_t)(slot0 + r) * plane + d0;
+        pack_split_store(XK + base + ((size_t)b * vp + c) * vk, xs, lane);
+        pack_split_store(XKT + base + ((size_t)c * vp + b) * vk, xs, lane);
     }
 }
 
 // blockIdx.x = q*v + x (x = b for T2K, x = c for T2KT), blockIdx.y = chunk of 64 along the contiguous source index y,
-// blockIdx.z = chunk of 64 along l.
+// blockIdx.z = chunk of 64 along l (two packed rows).
 __global__ void __launch_bounds__(256)
-pack_t2k_kernel(const double* __restrict__ t2, int v, int vp, int o, int ok, float* __restrict__ T2K,
-                float* __restrict__ T2KT, const float* __restrict__ scale_ptr) {
+pack_t2k_kernel(const double* __restrict__ t2, int v, int vp, int o, int ok, uint32_t* __restrict__ T2K,
+                uint32_t* __restrict__ T2KT, const float* __restrict__ scale_ptr) {
     const double scale = (double)*scale_ptr;
     __shared__ double tile[64][65];
     const int q = blockIdx.x / v, x = blockIdx.x % v;
     const int y0 = blockIdx.y * 64, l0 = blockIdx.z * 64;
     const int ny = min(64, v - y0), nl = min(64, o - l0);
-    for (int e = threadIdx.x; e < nl * ny; e += 256) {
+    for (int e = threadIdx.x; e < 64 * ny; e += 256) {
         const int l = e / ny, yy = e % ny;
-        tile[l][yy] = t2[(((size_t)q * o + l0 + l) * v + x) * v + y0 + yy];      // t2[q][l][x][y]
+        tile[l][yy] = l < nl ? t2[(((size_t)q * o + l0 + l) * v + x) * v + y0 + yy] : 0.0;      // t2[q][l][x][y]
     }
     __syncthreads();
-    for (int e = threadIdx.x; e < nl * ny; e += 256) {
-        const int l = e % nl, yy = e / nl;
-        const double val = tile[l][yy];
-        const float wd = (float)(val * scale);
-        T2K[(((size_t)q * v + x) * vp + (y0 + yy)) * ok + l0 + l] = wd;     // T2K [q][b=x][c=y][l]
-        T2KT[(((size_t)q * v + (y0 + yy)) * vp + x) * ok + l0 + l] = wd;    // T2KT[q][b=y][c=x][l] = t2[q][l][x][y]
+    const int lane = threadIdx.x & 31;
+    for (int e = threadIdx.x; e < 64 * ny; e += 256) {       // a warp = 32 consecutive l of one y
+        const int lh = (e >> 5) & 1, yy = e >> 6;
+        if (l0 + lh * 32 >= ok) continue;                    // warp-uniform
+        const float xs = (float)(tile[lh * 32 + lane][yy] * scale);
+        const int l = l0 + lh * 32;
+        pack_split_store(T2K + (((size_t)q * v + x) * vp + (y0 + yy)) * ok + l, xs, lane);     // T2K [q][b=x][c=y][l]
+        pack_split_store(T2KT + (((size_t)q * v + (y0 + yy)) * vp + x) * ok + l, xs, lane);    // T2KT[q][b=y][c=x][l]
+    }
+}
+
+// T2A[row][d], row = (p,q,a): one warp per (row, K chunk)
+__global__ void __launch_bounds__(256)
+pack_t2a_kernel(const double* __restrict__ t2, size_t rows, int v, int vk, uint32_t* __restrict__ T2A,
+                const float* __restrict__ scale_ptr) {
+    const double scale = (double)*scale_ptr;
+    const int lane = threadIdx.x & 31, nch = vk / 32;
+    const size_t nw = rows * nch;
+    for (size_t w = blockIdx.x * (size_t)8 + (threadIdx.x >> 5); w < nw; w += (size_t)gridDim.x * 8) {
+        const size_t row = w / nch;
+        const int d = (int)(w % nch) * 32 + lane;
+        const float xs = d < v ? (float)(t2[row * v + d] * scale) : 0.0f;
+        pack_split_store(T2A + row * vk + (d - lane), xs, lane);
+    }
+}
+
+// OtA[r][p][a][l] = -ovoo[p][a][l][r]: one warp per ((r,p,a), K chunk)
+__global__ void __launch_bounds__(256)
+pack_ota_kernel(const double* __restrict__ ovoo, int v, int o, int ok, uint32_t* __restrict__ OtA,
+                const float* __restrict__ scale_ptr) {
+    const double scale = (double)*scale_ptr;
+    const int lane = threadIdx.x & 31, nch = ok / 32;
+    const size_t nw = (size_t)o * o * v * nch;
+    for (size_t w = blockIdx.x * (size_t)8 + (threadIdx.x >> 5); w < nw; w += (size_t)gridDim.x * 8) {
+        const size_t row = w / nch;                        // (r, p, a)
+        const int l = (int)(w % nch) * 32 + lane;
+        const int a = (int)(row % v), p = (int)((row / v) % o), r = (int)(row / ((size_t)v * o));
+        const float xs = l < o ? (float)(-ovoo[(((size_t)p * v + a) * o + l) * o + r] * scale) : 0.0f;
+        pack_split_store(OtA + row * ok + (l - lane), xs, lane);
     }
 }
 

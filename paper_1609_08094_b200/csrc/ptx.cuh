@@ -61,6 +61,16 @@ __device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* m
         : "memory");
 }
 
+// Same load issued by either CTA of a CTA pair (cta_group::2): the completion bytes are signalled on the mbarrier at
+// the given shared::cluster address, which may live in the peer CTA (the pair's leader collects both CTAs' tiles).
+__device__ __forceinline__ void tma_load_3d_pair(void* smem_dst, const CUtensorMap* m, uint32_t bar_cluster_addr, int c0,
+                                                 int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar_cluster_addr), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+}
+
 // ---------------------------------------------------------------- thread-block clusters
 __device__ __forceinline__ uint32_t cluster_ctarank() {
     uint32_t r;
@@ -80,12 +90,6 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t cta_addr, uint32_t rank) {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster_addr) {
     asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
 }
-// Same with the default semantics of mbarrier.arrive (release at CTA scope) on a barrier that may live in the peer
-// CTA: orders the arriving thread's earlier shared-memory writes (already made visible to the async proxy by
-// fence.proxy.async) before the arrival, without the cluster-scope MEMBAR.
-__device__ __forceinline__ void mbar_arrive_cluster_release(uint32_t bar_cluster_addr) {
-    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
-}
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
@@ -104,7 +108,7 @@ __device__ __forceinline__ double lds_f64(uint32_t addr) {
     return v;
 }
 
-// ---------------------------------------------------------------- tcgen05 / TMEM (mixed path, gemm_tf32.cuh)
+// ---------------------------------------------------------------- tcgen05 / TMEM (mixed path, gemm_f16split.cuh)
 // TMEM addresses are (lane << 16 | column); the allocation's base is written to shared memory by the allocating warp.
 __device__ __forceinline__ void tc_fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -154,7 +158,6 @@ __device__ __forceinline__ void tmem_ld_32x32b_x16(uint32_t taddr, uint32_t (&r)
         : "r"(taddr)
         : "memory");
 }
-// Register re-partitioning between warpgroups (all four warps of a warpgroup execute the same instruction).
 // packed FP32 add (sm_100: FADD2), round to nearest: (acc.lo + a, acc.hi + b)
 __device__ __forceinline__ uint64_t fadd2_rn(uint64_t acc, uint32_t a, uint32_t b) {
     uint64_t r;
@@ -172,6 +175,7 @@ __device__ __forceinline__ void stg_v8(float* p, const float (&w)[8]) {
                  "f"(w[4]), "f"(w[5]), "f"(w[6]), "f"(w[7])
                  : "memory");
 }
+// Register re-partitioning between warpgroups (all four warps of a warpgroup execute the same instruction).
 template <int N> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }

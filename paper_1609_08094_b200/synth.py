@@ -125,6 +125,34 @@ def make_inputs_device(nocc: int, nvirt: int, naux: int, seed: int = 0, t1_sigma
     }
 
 
+def make_inputs_sliced(nocc: int, nvirt: int, naux: int, seed: int = 0, t1_sigma: float = 1e-3):
+    """Host inputs WITHOUT the full vvvo tensor (16-35 GB at configs[3..4]): the small tensors plus the B factors.
+
+    Returns (eps_o, eps_v, t1, t2, ovoo, ovov, B); any slice vvvo[:, :, :, r] follows from ``vvvo_slice``.
+    Same random draws and the same formulas as ``make_inputs``.
+    """
+    o, v = nocc, nvirt
+    eps_o, eps_v, B, t1 = draw_factors(o, v, naux, seed, t1_sigma)
+    Boo = np.ascontiguousarray(B[:, :o, :o]).reshape(naux, o * o)
+    Bov = np.ascontiguousarray(B[:, :o, o:]).reshape(naux, o * v)
+    ovoo = (Bov.T @ Boo).reshape(o, v, o, o)
+    ovov = (Bov.T @ Bov).reshape(o, v, o, v)
+    denom = (eps_o[:, None, None, None] + eps_o[None, :, None, None]
+             - eps_v[None, None, :, None] - eps_v[None, None, None, :])
+    t2 = np.ascontiguousarray(ovov.transpose(0, 2, 1, 3)) / denom
+    return (eps_o, eps_v, np.ascontiguousarray(t1), np.ascontiguousarray(t2), np.ascontiguousarray(ovoo),
+            np.ascontiguousarray(ovov), B)
+
+
+def vvvo_slice(B: np.ndarray, nocc: int, nvirt: int, r: int) -> np.ndarray:
+    """vvvo[:, :, :, r] = (ab|cr) = sum_Q B[Q,a,b] B[Q,c,r] as a C-ordered [v,v,v] array (generator only)."""
+    o, v = nocc, nvirt
+    naux = B.shape[0]
+    Bvv = np.ascontiguousarray(B[:, o:, o:]).reshape(naux, v * v)
+    Bvr = np.ascontiguousarray(B[:, o:, r])                       # [naux, v]
+    return np.ascontiguousarray((Bvv.T @ Bvr).reshape(v, v, v))
+
+
 def triplet_list(nocc: int):
     """Enumeration order of the restricted loop, i<=j<=k (Eq. (5.0.7b))."""
     return [(i, j, k) for i in range(nocc) for j in range(i, nocc) for k in range(j, nocc)]

@@ -39,7 +39,7 @@ def test_header_declares_the_survey_entry_points():
 def test_library_exports_every_declared_symbol(lib):
     for name in declared_functions():
         assert hasattr(lib, name), f"{name} declared in include/*.h but not exported"
-    assert binding.triples_abi_version() == 1
+    assert binding.triples_abi_version() == 2
 
 
 def test_binding_has_the_same_names():

@@ -1,0 +1,166 @@
+"""GPU tests of the SURVEY.md 8(f) rows built on the same kernels as triples_energy: out-of-core streaming of the
+(vv|vo) slices (NEXT-1), the RI-direct slice build (NEXT-2; Eq. (2.1.3)) and the
+triplet-sharded run (NEXT-3; L119-L121).  Each is compared with the CPU oracle and with the resident run."""
+import numpy as np
+import pytest
+import torch
+
+import paper_1609_08094_b200 as tb
+from oracle import oracle
+from paper_1609_08094_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL = {tb.FP64: 1e-10, tb.MIXED: 1e-5}
+STREAMED, RI = 1, 2
+
+
+def dev(inp):
+    return [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in inp.arrays()]
+
+
+def ws_bytes(n):
+    return torch.empty(n, dtype=torch.uint8, device="cuda")
+
+
+def resident(inp, prec):
+    o, v = inp.nocc, inp.nvirt
+    d = dev(inp)
+    et = torch.zeros((tb.triples_triplet_count(o), 3), dtype=torch.float64, device="cuda")
+    E = tb.triples_energy(o, v, *d, prec, ws_bytes(tb.triples_workspace_bytes(o, v, prec)), e_triplet_out=et)
+    return E, et.cpu().numpy(), d
+
+
+def slice_major_host(inp):
+    """vovv_host[k,a,b,c] = (ab|ck), pinned (the layout triples_energy_streamed reads; generator-side reshuffle)."""
+    t = torch.from_numpy(np.ascontiguousarray(inp.vvvo.transpose(3, 0, 1, 2))).pin_memory()
+    return t, t.numpy()
+
+
+@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED], ids=["fp64", "mixed"])
+@pytest.mark.parametrize("o,v,naux,win,extra", [(6, 24, 40, 1, 0), (7, 33, 40, 1, 1), (9, 40, 50, 2, 0), (14, 64, 70, 2, 2),
+                                                (5, 17, 30, 0, 0)])
+def test_streamed_is_bitwise_the_resident_run(o, v, naux, win, extra, prec):
+    """A device budget that holds only a few slices: per-triplet energies equal the resident path bit for bit."""
+    inp = synth.make_inputs(o, v, naux, seed=11, t1_sigma=0.2)
+    E, et, d = resident(inp, prec)
+    keep, host = slice_major_host(inp)
+    lo = tb.triples_workspace_bytes_streamed(o, v, prec, 0, win)
+    n0, _ = tb.triples_cache_slots(o, v, 0, prec, STREAMED, lo)
+    nbytes = tb.triples_workspace_bytes_streamed(o, v, prec, n0 + extra, win)
+    nslots, w = tb.triples_cache_slots(o, v, 0, prec, STREAMED, nbytes)
+    assert nslots == min(o, n0 + extra)
+    if nslots < o:
+        loads, _, _ = tb.triples_plan_slices(o, v, prec, STREAMED, nslots, w)
+        assert len(loads) > o                                  # slices really are evicted and re-loaded
+    ets = torch.zeros_like(torch.from_numpy(et)).cuda()
+    for absmax in ([0.0] if prec == tb.FP64 else [0.0, float(np.abs(inp.vvvo).max())]):
+        Es = tb.triples_energy_streamed(o, v, d[0], d[1], d[2], d[3], host, d[5], d[6], prec, ws_bytes(nbytes),
+                                        e_triplet_out=ets, vvvo_absmax=absmax)
+        assert Es == E
+        assert np.array_equal(ets.cpu().numpy(), et)
+    Eo = oracle.energy_restricted(o, v, *inp.arrays())
+    assert abs(E[0] - Eo[0]) <= TOL[prec] * abs(Eo[0])
+
+
+def test_streamed_profile_counts_slices_and_bytes():
+    o, v, naux = 9, 40, 50
+    inp = synth.make_inputs(o, v, naux, seed=2)
+    d = dev(inp)
+    keep, host = slice_major_host(inp)
+    nbytes = tb.triples_workspace_bytes_streamed(o, v, tb.FP64, 0, 1)
+    loads, _, info = tb.triples_plan_slices(o, v, tb.FP64, STREAMED, 0, 1)
+    tb.triples_set_profiling(True)
+    try:
+        tb.triples_energy_streamed(o, v, d[0], d[1], d[2], d[3], host, d[5], d[6], tb.FP64, ws_bytes(nbytes))
+        p = tb.triples_last_profile()
+    finally:
+        tb.triples_set_profiling(False)
+    assert p["slices_loaded"] == len(loads) and p["h2d_bytes"] == len(loads) * 8 * v ** 3
+
+
+@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED], ids=["fp64", "mixed"])
+@pytest.mark.parametrize("o,v,naux,slots", [(3, 5, 9, 0), (6, 24, 37, 0), (8, 40, 120, 0), (7, 33, 50, 7), (9, 48, 130, 4),
+                                            (5, 130, 40, 0)])
+def test_ri_direct_matches_the_oracle(o, v, naux, slots, prec):
+    """No vvvo tensor on the device: slices rebuilt from B.  Full E(T), E[4], E[5] and every triplet vs the oracle
+    (which is fed the B-built integrals of the same generator)."""
+    inp = synth.make_inputs(o, v, naux, seed=4, t1_sigma=0.3)
+    _, _, B, _ = synth.draw_factors(o, v, naux, seed=4, t1_sigma=0.3)
+    d = dev(inp)
+    Bd = torch.from_numpy(B).cuda()
+    nbytes = tb.triples_workspace_bytes_ri(o, v, naux, prec, slots, 0)
+    et = torch.zeros((tb.triples_triplet_count(o), 3), dtype=torch.float64, device="cuda")
+    tb.triples_set_profiling(True)
+    try:
+        E = tb.triples_energy_ri(o, v, naux, d[0], d[1], d[2], d[3], Bd, d[5], d[6], prec, ws_bytes(nbytes), e_triplet_out=et)
+        p = tb.triples_last_profile()
+    finally:
+        tb.triples_set_profiling(False)
+    (Eo, et_o) = oracle.energy_restricted(o, v, *inp.arrays(), with_triplets=True)
+    scale = abs(Eo[1])
+    for n in range(3):
+        assert abs(E[n] - Eo[n]) <= TOL[prec] * max(abs(Eo[n]), 1e-3 * scale), (n, E, Eo)
+    assert np.abs(et.cpu().numpy() - et_o).max() <= TOL[prec] * np.abs(et_o).max()
+    assert p["slices_loaded"] >= o - (1 if o == 1 else 0) and p["ri_flops"] == p["slices_loaded"] * 2.0 * naux * v ** 3
+    if prec == tb.FP64:       # same contraction kernels, operands equal up to the rounding order of the slice build
+        Er, etr, _ = resident(inp, prec)
+        assert abs(E[0] - Er[0]) <= 1e-12 * abs(Er[0])
+
+
+@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED], ids=["fp64", "mixed"])
+@pytest.mark.parametrize("o,v,naux,nshards", [(6, 24, 40, 2), (9, 40, 50, 3), (8, 40, 120, 8), (3, 9, 12, 5)])
+def test_sharded_partials_add_up_to_the_full_run(o, v, naux, nshards, prec):
+    inp = synth.make_inputs(o, v, naux, seed=8, t1_sigma=0.2)
+    E, et, d = resident(inp, prec)
+    ws = ws_bytes(tb.triples_workspace_bytes(o, v, prec))
+    _, sot, _ = tb.triples_plan_shards(o, v, prec, nshards)
+    tot = np.zeros(3)
+    seen = np.zeros_like(et)
+    for s in range(nshards):
+        ets = torch.zeros((len(et), 3), dtype=torch.float64, device="cuda")
+        part = tb.triples_energy_sharded(o, v, *d, prec, s, nshards, ws, e_triplet_out=ets)
+        ets = ets.cpu().numpy()
+        mine = sot == s
+        assert np.array_equal(ets[mine], et[mine]) and np.all(ets[~mine] == 0.0)     # bitwise the full run's rows
+        seen += ets
+        tot += np.array(part)                                                         # added in shard order
+    assert np.array_equal(seen, et)
+    for n in range(3):
+        assert abs(tot[n] - E[n]) <= 1e-13 * abs(E[1])
+
+
+def test_host_pointer_where_a_device_pointer_is_expected_is_einval():
+    """cudaPointerGetAttributes check (no sticky CUDA fault): the library stays usable afterwards."""
+    import ctypes
+    inp = synth.make_inputs(3, 8, 10, seed=0)
+    o, v = inp.nocc, inp.nvirt
+    d = dev(inp)
+    ws = ws_bytes(tb.triples_workspace_bytes(o, v, tb.FP64))
+    L = tb.binding.lib()
+    host_t2 = np.ascontiguousarray(inp.t2)
+    e_out = (ctypes.c_double * 3)()
+    ptrs = [ctypes.c_void_p(t.data_ptr()) for t in d]
+    ptrs[3] = ctypes.c_void_p(host_t2.ctypes.data)
+    rc = L.triples_energy(o, v, *ptrs, tb.FP64, ctypes.c_void_p(ws.data_ptr()), ws.numel(), None, e_out, None)
+    assert rc == 1 and b"not a device pointer" in L.triples_last_error()
+    E = tb.triples_energy(o, v, *d, tb.FP64, ws)
+    Eo = oracle.energy_restricted(o, v, *inp.arrays())
+    assert abs(E[0] - Eo[0]) <= 1e-10 * abs(Eo[0])
+
+
+def test_binding_rejects_wrong_sizes():
+    inp = synth.make_inputs(3, 8, 10, seed=0)
+    o, v = inp.nocc, inp.nvirt
+    d = dev(inp)
+    ws = ws_bytes(tb.triples_workspace_bytes(o, v, tb.FP64))
+    with pytest.raises(ValueError):
+        tb.triples_energy(v, o, *d, tb.FP64, ws)                      # swapped o / v
+    with pytest.raises(ValueError):
+        tb.triples_energy(o, v, *d, tb.FP64, ws, e_triplet_out=torch.zeros(5, dtype=torch.float64, device="cuda"))
+
+
+def test_fp64_peak_probe():
+    ws = ws_bytes(1 << 20)
+    tf = tb.triples_probe_fp64_peak(ws, iters=4000)
+    assert 20.0 < tf < 60.0, tf           # B200: 148 SM x 128 flop/clk x ~1.9 GHz = ~37 TFLOP/s
