@@ -8,9 +8,18 @@ A "step" is one pass of the whole hot path -- repack, every contraction batch, e
 the per-triplet finalize and the total -- i.e. one E(T) of the workload.  Prints ONE JSON line (rank 0).
 
 Metric: (T) TFLOP/s = T*(12 v^4 + 12 o v^3) / seconds per E(T), T = o(o+1)(o+2)/6 (Eq. (5.0.7b)),
-the paper's task count (i=j=k tasks included although they contribute zero and are skipped).
-Multi-GPU: the path is single-GPU by north_star ("replicas only"): --gpus N runs N independent
-replicas of the same workload, one process per GPU; no data-path collective.
+the paper's task count; `executed_value` counts the flops the kernels really execute (i=j=k tasks skipped,
+coinciding contractions of i=j / j=k tasks computed once) and is the figure to hold against the hardware peak.
+
+The default line (medium, FP64) also carries: the mixed-precision path on the same workload (`mixed_path`), the
+RI-direct and out-of-core variants (`ri_direct`, `streamed`), and short legs on the two largest single-GPU
+configs (`legs.large`: FP64 + mixed + streamed, `legs.largest`: mixed), each with its own roofline fractions
+and its parity against the stored oracle values of tests/golden/.  --no-legs / --no-variants skip them.
+
+Multi-GPU: north_star builds a single-GPU path ("replicas only"): --gpus N runs N
+independent replicas, one process per GPU, no data-path collective.  --sharded instead cuts the restricted loop
+into N contiguous ranges of window blocks (triples_energy_sharded) and adds the three partial sums of every rank in
+rank order: the triplet-sharded mode of SURVEY 8(f) NEXT-3 ("scaling": "strong").
 """
 from __future__ import annotations
 
@@ -29,7 +38,8 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 NAMES = ("eps_o", "eps_v", "t1", "t2", "vvvo", "ovoo", "ovov")
-FP64_DMMA_PEAK_TFLOPS = 37.0   # measured, profiles/r01_fp64_peak_probe.txt (148 SM x 128 flop/clk x 1.965 GHz = 37.2)
+MIXED_DTYPE = "fp16 split x = h + l (f32 accumulate), f64 reduction"
+GOLDEN_OF = {"small": "small_full", "medium": "medium_full", "large": "large_sample", "largest": "largest_sample"}
 
 
 def formula_flops(o: int, v: int) -> float:
@@ -65,6 +75,7 @@ class ClockSampler:
             self.thread.start()
         except OSError:
             self.proc = None
+        return self
 
     def _read(self):
         for line in self.proc.stdout:
@@ -105,6 +116,21 @@ def oracle_sample_seconds(host, trips):
     return time.perf_counter() - t0, e
 
 
+def oracle_c_loops_rate():
+    """The plain C-loop oracle (oracle/triples_oracle.c, no BLAS) on ONE triplet of configs[1] (small: a medium
+    triplet takes it close to a minute on one core; the loops over one ijk cycle are not threaded)."""
+    from oracle import oracle
+    from paper_1609_08094_b200 import synth
+
+    o, v, _ = synth.CONFIGS["small"]
+    inp = synth.make_config("small", seed=0)
+    t0 = time.perf_counter()
+    oracle.energy_subset(o, v, *inp.arrays(), [(0, 1, 2)])
+    dt = time.perf_counter() - t0
+    return {"value": (12.0 * v ** 4 + 12.0 * o * v ** 3) / dt / 1e12, "unit": "TFLOP/s", "cores": 1,
+            "kind": "oracle (plain C loops, oracle_triples_subset)", "sample": f"1 triplet (0,1,2) of small (16,120), {dt:.1f} s"}
+
+
 def blas_threads():
     try:
         from threadpoolctl import threadpool_info
@@ -130,6 +156,25 @@ def reduce_over_ranks(local_seconds: float, local_units: float, world: int):
     return float(t.item()), float(u.item())
 
 
+def combine_shard_partials(partial, world: int):
+    """Sharded mode: the only exchange step of the method -- all-gather of (E(T), E[4], E[5]) of every rank, added
+    in RANK ORDER on every rank (bitwise reproducible for a fixed world size)."""
+    if world == 1:
+        return tuple(float(x) for x in partial)
+    import torch
+    import torch.distributed as dist
+
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    mine = torch.tensor(list(partial), dtype=torch.float64, device=dev)
+    parts = [torch.zeros(3, dtype=torch.float64, device=dev) for _ in range(world)]
+    dist.all_gather(parts, mine)
+    tot = [0.0, 0.0, 0.0]
+    for p in parts:                       # rank order
+        for n in range(3):
+            tot[n] += float(p[n].item())
+    return tuple(tot)
+
+
 def run_reference(args, rank, world):
     """--impl reference: the oracle as it stands on the host cores, each step a bounded sample of the workload."""
     if rank != 0:
@@ -150,21 +195,171 @@ def run_reference(args, rank, world):
     flops = len(trips) * (12.0 * v ** 4 + 12.0 * o * v ** 3)
     value = flops / per_step / 1e12
     sample = f"{len(trips)} of {o*(o+1)*(o+2)//6} triplets per step ({trips}), oracle.energy_subset_numpy"
+    kind = "oracle (numpy restatement of Eq. (2.2.1)-(2.2.5), BLAS einsum)"
     line = {
         "impl": "reference", "metric": "(T) TFLOP/s", "value": value, "unit": "TFLOP/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": per_step * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(args, o, v, naux), "sample": sample},
+        "config": {"workload": workload_name(args.config, args.precision, o, v, naux), "sample": sample},
         "s_per_ET_extrapolated": formula_flops(o, v) / (value * 1e12),
-        "cpu_baseline": {"value": value, "unit": "TFLOP/s", "cores": blas_threads(), "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "TFLOP/s", "cores": blas_threads(), "kind": kind, "sample": sample},
         "e2e": {"value": value, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
 
 
-def workload_name(args, o, v, naux):
-    return f"{args.config}: nocc={o} nvirt={v} naux={naux} seed=0, {args.precision}, full E(T) over all i<=j<=k"
+def workload_name(config, precision, o, v, naux):
+    return f"{config}: nocc={o} nvirt={v} naux={naux} seed=0, {precision}, full E(T) over all i<=j<=k"
+
+
+def load_golden(config):
+    path = os.path.join(ROOT, "tests", "golden", GOLDEN_OF.get(config, "") + ".json")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        return json.load(f)
+
+
+def parity_vs_golden(config, et, triplet_index, tol):
+    """Largest deviation of the timed run's per-triplet energies from the oracle's stored values (tests/golden/,
+    written by tests/golden/make_golden.py from oracle/ only), relative to |w e4| of the triplet."""
+    g = load_golden(config)
+    if g is None or not g["triplets_ijk"]:
+        return None
+    want = np.array(g["energies"])
+    worst, n_cmp = 0.0, 0
+    for n, t in enumerate(g["triplets_ijk"]):
+        if t[0] == t[1] == t[2]:
+            continue
+        got = et[triplet_index[tuple(t)]]
+        worst = max(worst, abs(got[0] - want[n, 0]) / abs(want[n, 1]), abs(got[1] - want[n, 1]) / abs(want[n, 1]))
+        n_cmp += 1
+    return {"max_rel_err": worst, "triplets_compared": n_cmp, "tolerance": tol, "ok": bool(worst <= tol),
+            "source": f"tests/golden/{GOLDEN_OF[config]}.json ({g['mode']}; oracle values), against the timed run's e_triplet_out"}
+
+
+def rooflines(tb, prec, prof, peaks, peak_kind, fp64_peak, traffic):
+    """Contraction (tensor pipe) and fused reduction (HBM) rooflines from one profiled step."""
+    gemm_tflops = prof["contraction_flops"] / (prof["contraction_ms"] * 1e-3) / 1e12
+    red_gbs = prof["reduction_bytes"] / (prof["reduction_ms"] * 1e-3) / 1e9
+    step_ms = prof["prepare_ms"] + prof["contraction_ms"] + prof["reduction_ms"] + prof["other_ms"] + prof["slices_ms"]
+    nl = max(prof["contraction_launches"], 1)
+    if prec == tb.FP64:
+        kernel = "gemm_f64_kernel"
+        peak = fp64_peak["tflops"]
+        peak_note = fp64_peak["note"]
+    else:
+        kernel = "gemm_f16split_kernel"
+        peak = peaks["bf16_tflops_sustained"] * 0.5
+        peak_note = (f"FP32-class tensor rate = 0.5 x bf16 sustained cuBLAS ({peak_kind}, MEASURED_PEAKS.json; the guide's "
+                     "nominal tf32:bf16 ratio). achieved = ALGORITHMIC flops (4v^3(v+o) per executed contraction job); the "
+                     "split h*h' + h*l' + l*h' runs as three FP16 MMAs per product, i.e. 1.5x that many tf32-rate flops "
+                     "of tensor-pipe time: tensor_pipe_tf32_equiv / frac_tensor_pipe")
+    roof = {"bound": "tensor", "kernel": kernel, "achieved": gemm_tflops, "peak": peak, "unit": "TFLOP/s",
+            "frac": gemm_tflops / peak, "traffic": None, "peak_note": peak_note,
+            "share_of_step": prof["contraction_ms"] / step_ms, "launches_per_step": prof["contraction_launches"],
+            "flops_per_launch": prof["contraction_flops"] / nl, "avg_launch_ms": prof["contraction_ms"] / nl}
+    if prec != tb.FP64:
+        roof["tensor_pipe_tf32_equiv"] = 1.5 * gemm_tflops
+        roof["frac_tensor_pipe"] = 1.5 * gemm_tflops / peak
+    nr = max(prof["reduction_launches"], 1)
+    red = {"bound": "hbm", "kernel": "reduce_kernel<double>" if prec == tb.FP64 else "reduce_kernel<float>",
+           "achieved": red_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": red_gbs / peaks["hbm_gbs"],
+           "traffic": None,
+           "peak_note": f"{peak_kind} copy bandwidth (read + write); the reduction only reads, and a pure read stream "
+                        "can run a few per cent above a copy, so a frac slightly above 1 is a denominator mismatch, "
+                        "not skipped work",
+           "bytes_per_launch": prof["reduction_bytes"] / nr, "avg_launch_ms": prof["reduction_ms"] / nr}
+    for r in (roof, red):
+        t = (traffic or {}).get(r["kernel"])
+        if t:
+            r["traffic"] = t["dram_bytes"]
+            r["traffic_note"] = t["note"]
+        else:
+            r["traffic_note"] = "no ncu --set full capture of this kernel at this config this round (profiles/)"
+    return roof, red
+
+
+def load_traffic(config):
+    path = os.path.join(ROOT, "profiles", "r02_ncu_traffic.json")
+    if not os.path.exists(path):
+        return {}
+    with open(path) as f:
+        return json.load(f).get(config, {})
+
+
+def timed_steps(fn, steps, warmup, stream, torch):
+    """`warmup` untimed calls, then `steps` calls between CUDA events on `stream`; seconds per step and last result."""
+    out = None
+    for _ in range(warmup):
+        out = fn()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(steps):
+        out = fn()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / 1e3 / steps, out
+
+
+def profiled_step(tb, fn):
+    tb.triples_set_profiling(True)
+    try:
+        fn()
+        return tb.triples_last_profile()
+    finally:
+        tb.triples_set_profiling(False)
+
+
+def precision_leg(tb, torch, config, prec, o, v, dargs, ws, stream, steps, warmup, peaks, peak_kind, fp64_peak, index):
+    """One precision of one config: whole-step rate, rooflines of the two dominant kernels, parity vs goldens."""
+    T = tb.triples_triplet_count(o)
+    et = torch.zeros((T, 3), dtype=torch.float64, device="cuda")
+    sampler = ClockSampler(torch.cuda.current_device()).start()
+    sec, E = timed_steps(lambda: tb.triples_energy(o, v, *dargs, prec, ws, stream=stream, e_triplet_out=et), steps, warmup,
+                         stream, torch)
+    clocks = sampler.stop()
+    prof = profiled_step(tb, lambda: tb.triples_energy(o, v, *dargs, prec, ws, stream=stream))
+    roof, red = rooflines(tb, prec, prof, peaks, peak_kind, fp64_peak, load_traffic(config))
+    tol = 1e-10 if prec == tb.FP64 else 1e-5
+    leg = {"value": formula_flops(o, v) / sec / 1e12, "executed_value": prof["contraction_flops"] / sec / 1e12,
+           "unit": "TFLOP/s", "s_per_ET": sec, "steps": steps, "warmup": warmup,
+           "dtype": "f64" if prec == tb.FP64 else MIXED_DTYPE, "E_T": E[0], "E4": E[1], "E5": E[2],
+           "roofline": roof, "roofline_reduction": red, "clocks": clocks,
+           "parity": parity_vs_golden(config, et.cpu().numpy(), index, tol)}
+    return leg, E
+
+
+def streamed_leg(tb, torch, o, v, d, prec, stream, nslots, win, resident_sec, E_resident):
+    """Out-of-core run (NEXT-1): vvvo in pinned host memory (slice-major), a device cache of `nslots` slices; the
+    H2D copies of the slices are inside the timed region.  One warm-up-free timed call (the copies ARE the point)."""
+    vv = d["vvvo"]
+    host = torch.empty((o, v, v, v), dtype=torch.float64, pin_memory=True)
+    for k in range(o):                                  # generator-side reshuffle to the slice-major layout
+        host[k].copy_(vv[:, :, :, k])
+    torch.cuda.synchronize()
+    absmax = float(vv.abs().max().item()) if prec == tb.MIXED else 0.0
+    nbytes = tb.triples_workspace_bytes_streamed(o, v, prec, nslots, win)
+    slots, w = tb.triples_cache_slots(o, v, 0, prec, 1, nbytes)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    call = lambda: tb.triples_energy_streamed(o, v, d["eps_o"], d["eps_v"], d["t1"], d["t2"], host.numpy(), d["ovoo"],
+                                              d["ovov"], prec, ws, stream=stream, vvvo_absmax=absmax)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    E = call()
+    torch.cuda.synchronize()
+    sec = time.perf_counter() - t0
+    prof = profiled_step(tb, call)
+    del ws, host
+    return {"api": "triples_energy_streamed (C ABI; vovv_host pinned, slice-major)", "value": formula_flops(o, v) / sec / 1e12,
+            "unit": "TFLOP/s", "s_per_ET": sec, "cache_slots": slots, "slices": o, "window": w,
+            "device_workspace_bytes": nbytes, "vvvo_bytes": 8 * v ** 3 * o,
+            "h2d_bytes_per_step": prof["h2d_bytes"] + 8 * (o + v + o * v), "slices_loaded": prof["slices_loaded"],
+            "vs_resident": resident_sec / sec, "bitwise_equal_to_resident": bool(E == E_resident),
+            "note": "copies of batch b+2 run on a copy stream while batch b+1 computes; vs_resident = resident s / streamed s "
+                    "(1.0 = transfer fully hidden)"}
 
 
 def main():
@@ -181,6 +376,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-mixed-leg", action="store_true",
                     help="FP64 runs only: skip the extra mixed-precision measurement reported under 'mixed_path'")
+    ap.add_argument("--no-variants", action="store_true", help="skip the RI-direct and streamed measurements")
+    ap.add_argument("--no-legs", action="store_true", help="skip the short legs on the large / largest configs")
+    ap.add_argument("--sharded", action="store_true", help="--gpus N: triplet-sharded run instead of N replicas")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -205,16 +403,20 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     prec = tb.FP64 if args.precision == "fp64" else tb.MIXED
+    tol = 1e-10 if prec == tb.FP64 else 1e-5
     o, v, naux = synth.CONFIGS[args.config]
+    default_line = args.config == "medium" and prec == tb.FP64 and world == 1
     # ---- synthetic inputs: host copies (pinned, for the e2e leg and the oracle) and device-resident copies
     need_host = (not args.no_e2e) or (rank == 0 and not args.no_cpu_baseline)
     if need_host and args.config in ("tiny", "small", "medium"):
         inp = synth.make_config(args.config, seed=0)
         host = dict(zip(NAMES, inp.arrays()))
         dev = {k: torch.from_numpy(a).cuda() for k, a in host.items()}
+        B_host = None
     else:
         d = synth.make_inputs_device(o, v, naux, seed=0)
         dev = {k: d[k] for k in NAMES}
+        B_host = d["B_host"]
         host = None
         if need_host:
             host = {k: dev[k].cpu().numpy() for k in NAMES}
@@ -225,6 +427,8 @@ def main():
         ws_bytes = max(ws_bytes, tb.triples_workspace_bytes(o, v, tb.MIXED))
     ws = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
+    T = tb.triples_triplet_count(o)
+    index = {t: n for n, t in enumerate(synth.triplet_list(o))}
 
     def barrier():
         if world > 1:
@@ -233,82 +437,58 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # ---- roofline denominators measured in this run / on this pool
+    peaks, peak_kind = measured_peaks()
+    fp64_peak = {"tflops": tb.triples_probe_fp64_peak(ws, stream=stream),
+                 "note": "FP64 tensor-core (DMMA) peak measured in this run on this device with a register-resident "
+                         "mma.sync.m8n8k4.f64 loop on all SMs (triples_probe_fp64_peak, best of 3; 148 SM x 128 flop/clk "
+                         "x 1.965 GHz = 37.2)"}
+
     # ---- device-resident timing: W warm-up steps, then exactly K steps between CUDA events
+    sharded = args.sharded and world > 1
+    et = torch.zeros((T, 3), dtype=torch.float64, device="cuda")
+
+    def step():
+        if sharded:
+            part = tb.triples_energy_sharded(o, v, *dargs, prec, rank, world, ws, stream=stream, e_triplet_out=et)
+            return combine_shard_partials(part, world)
+        return tb.triples_energy(o, v, *dargs, prec, ws, stream=stream, e_triplet_out=et)
+
     tb.triples_set_profiling(False)
     E = None
     for _ in range(args.warmup):
-        E = tb.triples_energy(o, v, *dargs, prec, ws, stream=stream)
+        E = step()
     sampler = ClockSampler(local_rank)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     sampler.start()
     ev0.record(stream)
     for _ in range(args.steps):
-        E = tb.triples_energy(o, v, *dargs, prec, ws, stream=stream)
+        E = step()
     ev1.record(stream)
     barrier()
     clocks = sampler.stop()
     launches = tb.triples_last_launch_count() * args.steps
     sec = ev0.elapsed_time(ev1) / 1e3
-    sec_max, flops_all = reduce_over_ranks(sec, formula_flops(o, v) * args.steps, world)
+    units = formula_flops(o, v) * args.steps
+    sec_max, flops_all = reduce_over_ranks(sec, units / world if sharded else units, world)
     value = flops_all / sec_max / 1e12
     ms_per_step = sec_max / args.steps * 1e3
+    et_timed = et.cpu().numpy()
 
     # ---- per-kernel roofline: one extra profiled step (CUDA events around every launch, on the same stream)
-    tb.triples_set_profiling(True)
-    tb.triples_energy(o, v, *dargs, prec, ws, stream=stream)
-    prof = tb.triples_last_profile()
-    tb.triples_set_profiling(False)
-    peaks, peak_kind = measured_peaks()
-    gemm_tflops = prof["contraction_flops"] / (prof["contraction_ms"] * 1e-3) / 1e12
-    red_gbs = prof["reduction_bytes"] / (prof["reduction_ms"] * 1e-3) / 1e9
-    if prec == tb.FP64:
-        peak, peak_note = FP64_DMMA_PEAK_TFLOPS, ("FP64 DMMA peak measured on this pool's B200 with a register-resident "
-                                                  "mma.sync.m8n8k4.f64 loop (profiles/r01_fp64_peak_probe.txt)")
-    else:
-        peak = peaks["bf16_tflops_sustained"] * 0.5
-        peak_note = (f"TF32 dense = 0.5 x bf16 sustained cuBLAS ({peak_kind}, MEASURED_PEAKS.json; nominal ratio of the "
-                     "profiling guide). achieved = ALGORITHMIC flops (12v^4+12ov^3 per executed job triple); the split "
-                     "h*h' + h*l' + l*h' runs as three FP16 MMAs (K=16), i.e. 1.5x that many TF32-rate flops of "
-                     "tensor-pipe time: see tensor_pipe_tf32_equiv / frac_tensor_pipe")
-    roofline = {
-        "bound": "tensor", "kernel": "gemm_f64_kernel" if prec == tb.FP64 else "gemm_tf32_kernel",
-        "achieved": gemm_tflops, "peak": peak, "unit": "TFLOP/s", "frac": gemm_tflops / peak, "traffic": None,
-        "peak_note": peak_note,
-        "share_of_step": prof["contraction_ms"] / (prof["prepare_ms"] + prof["contraction_ms"] + prof["reduction_ms"] +
-                                                   prof["other_ms"]),
-        "launches_per_step": prof["contraction_launches"],
-        "flops_per_launch": prof["contraction_flops"] / max(prof["contraction_launches"], 1),
-        "avg_launch_ms": prof["contraction_ms"] / max(prof["contraction_launches"], 1),
-    }
-    if prec != tb.FP64:
-        roofline["tensor_pipe_tf32_equiv"] = 1.5 * gemm_tflops
-        roofline["frac_tensor_pipe"] = 1.5 * gemm_tflops / peak
-    roofline_reduction = {
-        "bound": "hbm", "kernel": "reduce_kernel", "achieved": red_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-        "frac": red_gbs / peaks["hbm_gbs"], "traffic": None, "peak_note": f"{peak_kind} copy bandwidth",
-        "bytes_per_launch": prof["reduction_bytes"] / max(prof["reduction_launches"], 1),
-        "avg_launch_ms": prof["reduction_ms"] / max(prof["reduction_launches"], 1),
-    }
-
-    # DRAM traffic per launch of the captured batch (ncu --set full summary committed under profiles/; medium only)
-    tpath = os.path.join(ROOT, "profiles", "r01_ncu_traffic.json")
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            tr = json.load(f).get(args.config, {})
-        g = tr.get(roofline["kernel"])
-        r = tr.get("reduce_kernel<double>" if prec == tb.FP64 else "reduce_kernel<float>")
-        if g:
-            roofline["traffic"] = g["dram_bytes"]
-            roofline["traffic_note"] = (f"ncu dram bytes of one captured launch ({g.get('jobs_in_launch')} jobs, "
-                                        "profiles/r01_ncu_full_medium.md); launches differ in size")
-        if r:
-            roofline_reduction["traffic"] = r["dram_bytes"]
-            roofline_reduction["traffic_note"] = "ncu dram bytes of one captured launch (profiles/r01_ncu_full_medium.md)"
+    prof = profiled_step(tb, step)
+    roofline, roofline_reduction = rooflines(tb, prec, prof, peaks, peak_kind, fp64_peak, load_traffic(args.config))
+    executed_local = prof["contraction_flops"] / (sec / args.steps) / 1e12
+    _, executed_value = reduce_over_ranks(sec, executed_local, world)
+    if not sharded and world > 1:
+        pass                                             # replicas: the sum over ranks is the whole-job rate
+    if prec == tb.FP64:                                  # sanity: executed work cannot beat the measured peak
+        assert executed_local <= 1.02 * fp64_peak["tflops"], (executed_local, fp64_peak)
 
     # ---- end-to-end: host (pinned) inputs through triples_energy_host, copies inside the timed region
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not sharded:
         pinned = {k: torch.from_numpy(np.ascontiguousarray(host[k])).pin_memory() for k in NAMES}
         hargs = [pinned[k].numpy() for k in NAMES]
         h2d = int(sum(a.nbytes for a in hargs))
@@ -324,72 +504,121 @@ def main():
         e2e = {"value": flops_e / sec_e_max / 1e12, "unit": "TFLOP/s", "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": 24, "s_per_ET": sec_e_max / args.steps,
                "api": "triples_energy_host (C ABI, host buffers pinned)"}
+        del pinned, hargs
 
     # ---- the paper's other precision beside the headline one (its single/double study): same workload
     mixed = None
     if mixed_leg:
-        tb.triples_energy(o, v, *dargs, tb.MIXED, ws, stream=stream)            # warm-up
-        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        m0.record(stream)
-        for _ in range(args.steps):
-            Em = tb.triples_energy(o, v, *dargs, tb.MIXED, ws, stream=stream)
-        m1.record(stream)
-        torch.cuda.synchronize()
-        msec = m0.elapsed_time(m1) / 1e3 / args.steps
-        tb.triples_set_profiling(True)
-        tb.triples_energy(o, v, *dargs, tb.MIXED, ws, stream=stream)
-        mp = tb.triples_last_profile()
-        tb.triples_set_profiling(False)
-        mg = mp["contraction_flops"] / (mp["contraction_ms"] * 1e-3) / 1e12
-        mr = mp["reduction_bytes"] / (mp["reduction_ms"] * 1e-3) / 1e9
-        tf32_peak = peaks["bf16_tflops_sustained"] * 0.5
-        mixed = {"value": formula_flops(o, v) / msec / 1e12, "unit": "TFLOP/s", "s_per_ET": msec,
-                 "dtype": "fp16 split x = h + l (f32 accumulate), f64 reduction",
-                 "E_T": Em[0], "E4": Em[1], "E5": Em[2],
-                 "rel_dev_from_fp64": {"E_T": abs(Em[0] - E[0]) / abs(E[0]), "E4": abs(Em[1] - E[1]) / abs(E[1]),
-                                       "E5_abs_dev_over_abs_E4": abs(Em[2] - E[2]) / abs(E[1]),
-                                       "note": "tolerance 1e-5 on E(T); E5 is 1e-7..1e-4 of E4 with the generator's "
-                                               "t1 ~ N(0,1e-3^2) and a sum of both signs, so its deviation is "
-                                               "given on the scale of E4 (tests pin E5 with t1 ~ N(0,1))"},
-                 "contraction": {"kernel": "gemm_tf32_kernel", "achieved": mg, "peak": tf32_peak, "unit": "TFLOP/s",
-                                 "frac": mg / tf32_peak, "frac_tensor_pipe": 1.5 * mg / tf32_peak,
-                                 "peak_note": "0.5 x measured sustained bf16; frac = algorithmic flops, "
-                                              "frac_tensor_pipe = TF32-rate-equivalent tensor work (DESIGN.md 7.2)"},
-                 "reduction": {"kernel": "reduce_kernel<float>", "achieved": mr, "peak": peaks["hbm_gbs"],
-                               "unit": "GB/s", "frac": mr / peaks["hbm_gbs"]}}
+        mixed, Em = precision_leg(tb, torch, args.config, tb.MIXED, o, v, dargs, ws, stream, args.steps, 1, peaks,
+                                  peak_kind, fp64_peak, index)
+        mixed["rel_dev_from_fp64"] = {
+            "E_T": abs(Em[0] - E[0]) / abs(E[0]), "E4": abs(Em[1] - E[1]) / abs(E[1]),
+            "E5_abs_dev_over_abs_E4": abs(Em[2] - E[2]) / abs(E[1]),
+            "note": "tolerance 1e-5 on E(T); E5 is 1e-7..1e-4 of E4 with the generator's t1 ~ N(0,1e-3^2) and a sum of both "
+                    "signs, so its deviation is given on the scale of E4 (tests pin E5 with t1 ~ N(0,1))"}
 
     # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample (rank 0, N=1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         trips = [t for t in synth.sample_triplets(o, 16, seed=0) if not (t[0] == t[1] == t[2])][: args.cpu_triplets]
         dt, e_or = oracle_sample_seconds(host, trips)
-        e_gpu = tb.triples_energy_subset(o, v, *dargs, prec, trips, ws, stream=stream)
-        tol = 1e-10 if prec == tb.FP64 else 1e-5
+        e_gpu = et_timed[[index[t] for t in trips]]            # the TIMED run's per-triplet energies
         parity = float(np.max(np.abs(e_gpu[:, 0] - e_or[:, 0]) / np.abs(e_or[:, 1])))
         cpu_flops = len(trips) * (12.0 * v ** 4 + 12.0 * o * v ** 3)
-        cpu = {"value": cpu_flops / dt / 1e12, "unit": "TFLOP/s", "cores": blas_threads(), "kind": "oracle",
-               "sample": f"{len(trips)} of {o*(o+1)*(o+2)//6} triplets ({trips}) via oracle.energy_subset_numpy, "
+        cpu = {"value": cpu_flops / dt / 1e12, "unit": "TFLOP/s", "cores": blas_threads(),
+               "kind": "oracle (numpy restatement of Eq. (2.2.1)-(2.2.5), BLAS einsum)",
+               "sample": f"{len(trips)} of {T} triplets ({trips}) via oracle.energy_subset_numpy, "
                          f"{dt:.1f} s; full E(T) extrapolated {formula_flops(o, v)/(cpu_flops/dt):.0f} s",
-               "parity_max_rel_err_on_sample": parity, "parity_ok": bool(parity <= tol)}
+               "parity_max_rel_err_on_sample": parity, "parity_ok": bool(parity <= tol),
+               "parity_source": "the timed run's e_triplet_out against the oracle run here",
+               "c_loops": oracle_c_loops_rate()}
+    parity_golden = parity_vs_golden(args.config, et_timed, index, tol) if rank == 0 else None
+
+    # ---- SURVEY 8(f) variants on the same workload: RI-direct slices (NEXT-2) and out-of-core slices (NEXT-1)
+    ri = streamed = None
+    if default_line and not args.no_variants:
+        if B_host is None:
+            _, _, B_host, _ = synth.draw_factors(o, v, naux, seed=0)
+        Bd = torch.from_numpy(B_host).cuda()
+        nb_ri = tb.triples_workspace_bytes_ri(o, v, naux, prec, o, 0)
+        ws_ri = ws if nb_ri <= ws.numel() else torch.empty(nb_ri, dtype=torch.uint8, device="cuda")
+        call = lambda: tb.triples_energy_ri(o, v, naux, dev["eps_o"], dev["eps_v"], dev["t1"], dev["t2"], Bd, dev["ovoo"],
+                                            dev["ovov"], prec, ws_ri, stream=stream)
+        sec_ri, Eri = timed_steps(call, 1, 1, stream, torch)
+        pri = profiled_step(tb, call)
+        ri = {"api": "triples_energy_ri (C ABI; B[naux,n,n] instead of vvvo)", "value": formula_flops(o, v) / sec_ri / 1e12,
+              "unit": "TFLOP/s", "s_per_ET": sec_ri, "naux": naux, "cache_slots": o,
+              "slices_built": pri["slices_loaded"], "ri_flops": pri["ri_flops"], "ri_ms": pri["slices_ms"],
+              "ri_flops_over_contraction_flops": pri["ri_flops"] / pri["contraction_flops"],
+              "device_workspace_bytes": nb_ri, "input_bytes_B": int(B_host.nbytes), "vvvo_bytes_not_needed": 8 * v ** 3 * o,
+              "rel_dev_from_resident": abs(Eri[0] - E[0]) / abs(E[0]),
+              "note": "value counts the method's flops T(12v^4+12ov^3); the slice GEMMs (2 naux v^3 each) are extra work, "
+                      "listed as ri_flops; a full cache builds every slice once"}
+        del Bd, ws_ri
+        d_ = dict(dev)
+        streamed = streamed_leg(tb, torch, o, v, d_, prec, stream, 12, 2, sec / args.steps, E)
+
+    # ---- short legs on the two largest single-GPU configs (the driver times only this default command)
+    legs = None
+    if default_line and not args.no_legs:
+        legs = {}
+        del dargs, dev, ws, et
+        host = None
+        import gc
+        for cfg, precs in (("large", (tb.FP64, tb.MIXED)), ("largest", (tb.MIXED,))):
+            gc.collect()
+            torch.cuda.empty_cache()
+            lo, lv, lnaux = synth.CONFIGS[cfg]
+            t0 = time.perf_counter()
+            d = synth.make_inputs_device(lo, lv, lnaux, seed=0)
+            torch.cuda.synchronize()
+            gen_s = time.perf_counter() - t0
+            largs = [d[k] for k in NAMES]
+            lws = torch.empty(max(tb.triples_workspace_bytes(lo, lv, p) for p in precs), dtype=torch.uint8, device="cuda")
+            lindex = {t: n for n, t in enumerate(synth.triplet_list(lo))}
+            leg = {"workload": workload_name(cfg, "+".join("fp64" if p == tb.FP64 else "mixed" for p in precs), lo, lv, lnaux),
+                   "input_generation_s": gen_s}
+            for p in precs:
+                key = "fp64" if p == tb.FP64 else "mixed"
+                leg[key], El = precision_leg(tb, torch, cfg, p, lo, lv, largs, lws, stream, 1 if p == tb.FP64 else 2, 1,
+                                             peaks, peak_kind, fp64_peak, lindex)
+                if cfg == "large" and p == tb.FP64 and not args.no_variants:
+                    del lws
+                    torch.cuda.empty_cache()
+                    leg["streamed_fp64"] = streamed_leg(tb, torch, lo, lv, d, p, stream, 16, 2, leg[key]["s_per_ET"], El)
+                    lws = torch.empty(max(tb.triples_workspace_bytes(lo, lv, q) for q in precs), dtype=torch.uint8,
+                                      device="cuda")
+            legs[cfg] = leg
+            del d, largs, lws
 
     if rank == 0:
         line = {
-            "metric": "(T) TFLOP/s", "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "s_per_ET": ms_per_step / 1e3,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64" if prec == tb.FP64 else "fp16 split x = h + l (f32 accumulate), f64 reduction", "data": "synthetic",
-            "config": {"workload": workload_name(args, o, v, naux), "parallelism": f"replicas x{world}",
+            "metric": "(T) TFLOP/s", "value": value, "executed_value": executed_value, "unit": "TFLOP/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "s_per_ET": ms_per_step / 1e3,
+            "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
+            "dtype": "f64" if prec == tb.FP64 else MIXED_DTYPE, "data": "synthetic",
+            "config": {"workload": workload_name(args.config, args.precision, o, v, naux),
+                       "parallelism": (f"triplet-sharded x{world}" if sharded else f"replicas x{world}"),
                        "l2": f"inputs larger than L2 (vvvo {8*v**3*o/1e6:.0f} MB, U buffers re-written every batch)",
-                       "flop_count": "T*(12v^4+12ov^3), T=o(o+1)(o+2)/6 (paper's task count, Eq. 5.0.7b)"},
+                       "flop_count": "value: T*(12v^4+12ov^3), T=o(o+1)(o+2)/6 (paper's task count, Eq. 5.0.7b); "
+                                     "executed_value: flops the kernels execute (i=j=k skipped, coinciding jobs once)",
+                       "why_this_config": "medium is the largest config whose FP64 step (3.1 s) fits the driver's "
+                                          "--steps 20 --warmup 5 protocol (47 FP64 steps incl. the e2e leg); large / "
+                                          "largest are timed as short legs of the same command (legs)"},
             "E_T": E[0], "E4": E[1], "E5": E[2],
             "clocks": clocks, "gpu_launches": int(launches),
             "roofline": roofline, "roofline_reduction": roofline_reduction,
             "phase_ms": {k: prof[k] for k in ("prepare_ms", "contraction_ms", "reduction_ms", "other_ms")},
-            "e2e": e2e, "cpu_baseline": cpu,
+            "parity": parity_golden, "e2e": e2e, "cpu_baseline": cpu,
         }
         if mixed is not None:
             line["mixed_path"] = mixed
+        if ri is not None:
+            line["ri_direct"] = ri
+        if streamed is not None:
+            line["streamed"] = streamed
+        if legs is not None:
+            line["legs"] = legs
         print(json.dumps(line), flush=True)
     if world > 1:
         import torch.distributed as dist

@@ -165,7 +165,12 @@ gemm_f16split_kernel(const __grid_constant__ SplitMaps maps, const GemmJob* __re
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------------------------------ MMA issuer
-        if (lane == 0 && rank == 0) {
+        // The WHOLE warp of the leader CTA walks the loop (convergent, so descriptors and loop state stay in uniform
+        // registers); one elected lane issues.  With a lone thread in a divergent branch the compiler moved every
+        // descriptor through ELECT + R2UR.BROADCAST -- ~26 dependent instructions per MMA, more than the 120 clk an
+        // MMA takes: the issue thread, not the tensor pipe, set the pace (ncu: pipe 44 % active, no role waiting).
+        if (rank == 0) {
+            const bool issuer = elect_one();
             const uint32_t idesc = umma_idesc_f16_m256((uint32_t)bn, 0, 0);   // FP16 x FP16 -> FP32
             const uint32_t smem_base = smem_u32(smem);
             uint32_t it = 0, chain = 0;
@@ -177,33 +182,32 @@ gemm_f16split_kernel(const __grid_constant__ SplitMaps maps, const GemmJob* __re
                     else if (c < 2 * nch_v) left = v - (c - nch_v) * FS_BK;
                     else if (c < 2 * nch_v + nch_o) left = o - (c - 2 * nch_v) * FS_BK;
                     else left = o - (c - 2 * nch_v - nch_o) * FS_BK;
-                    const int nk16 = left >= FS_BK ? 2 : (left + 15) >> 4;
+                    const bool two = left > 16;                           // K steps of 16 that carry data: 2 or 1
                     const uint32_t buf = chain & 1;
                     const bool first = (c % FS_CHAIN) == 0, last = (c % FS_CHAIN) == FS_CHAIN - 1 || c == nch - 1;
-                    if (first) {
-                        mbar_wait(&tempty[buf], ((chain >> 1) & 1) ^ 1);
-                        tc_fence_after_sync();
-                    }
+                    if (first) mbar_wait(&tempty[buf], ((chain >> 1) & 1) ^ 1);
                     mbar_wait(&full[s], (it / S) & 1);
                     tc_fence_after_sync();
-                    const uint32_t tacc = tmem_base + buf * 256;
-                    const uint32_t pM = smem_base + s * tile_bytes, pN = pM + FS_BM * 128;
-                    const uint64_t ml = umma_desc_sw128(pM), nl = umma_desc_sw128(pN);
-                    uint32_t acc = first ? 0u : 1u;
-                    // packed row: bytes 0..63 = 32 FP16 of h, 64..127 = 32 FP16 of l; K = 16 per MMA.  Cross terms
-                    // l*h' + h*l' first (small), then the main term h*h'
-                    for (int k = 0; k < nk16; ++k) {
-                        const uint64_t adv = (uint64_t)(k * 2);          // 32 bytes per k-step, in 16-byte units
-                        umma_f16_pair(tacc, ml + 4 + adv, nl + adv, idesc, acc);   // l * h'
-                        acc = 1;
-                        umma_f16_pair(tacc, ml + adv, nl + 4 + adv, idesc, 1);     // h * l'
+                    if (issuer) {
+                        const uint32_t tacc = tmem_base + buf * 256;
+                        // low descriptor words of the packed M / N tiles; bytes 0..63 of a row = 32 FP16 of h,
+                        // 64..127 = 32 FP16 of l; one K step = 32 bytes = 2 units of 16 bytes
+                        const uint32_t m = umma_desc_lo(smem_base + s * tile_bytes);
+                        const uint32_t n = umma_desc_lo(smem_base + s * tile_bytes + FS_BM * 128);
+                        // cross terms l*h' + h*l' first (small), then the main term h*h'
+                        umma_f16_pair(tacc, m + 4, n, idesc, first ? 0u : 1u);
+                        umma_f16_pair(tacc, m, n + 4, idesc, 1u);
+                        if (two) {
+                            umma_f16_pair(tacc, m + 6, n + 2, idesc, 1u);
+                            umma_f16_pair(tacc, m + 2, n + 6, idesc, 1u);
+                        }
+                        umma_f16_pair(tacc, m, n, idesc, 1u);
+                        if (two) umma_f16_pair(tacc, m + 2, n + 2, idesc, 1u);
+                        umma_commit_pair(&empty[s]);                       // both CTAs' ring slots
+                        if (last) umma_commit_pair(&tfull[buf]);           // both CTAs' accumulator warps
                     }
-                    for (int k = 0; k < nk16; ++k) {
-                        const uint64_t adv = (uint64_t)(k * 2);
-                        umma_f16_pair(tacc, ml + adv, nl + adv, idesc, 1);         // h * h'
-                    }
-                    umma_commit_pair(&empty[s]);                       // both CTAs' ring slots
-                    if (last) { umma_commit_pair(&tfull[buf]); ++chain; }   // both CTAs' accumulator warps
+                    __syncwarp();
+                    if (last) ++chain;
                 }
             }
         }

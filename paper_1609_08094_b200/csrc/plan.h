@@ -200,7 +200,7 @@ inline bool make_plan(int o, int v, int prec, Plan& P, int mode = SLICES_RESIDEN
         P.off_t2k = take(P.n_t2k * P.esz);
         P.off_t2kt = take(P.n_t2k * P.esz);
     }
-    if (P.nstage) P.off_stage = take((size_t)P.nstage * v * v * v * 8);
+    if (P.nstage) P.off_stage = take((size_t)P.nstage * v * v * P.vp * 8);
     if (mode == SLICES_RI) {
         P.off_bt = take((size_t)v * v * P.nauxp * 8);
         P.off_bo = take((size_t)o * naux * P.vp * 8);
@@ -307,12 +307,13 @@ inline void build_batches(const Plan& P, const std::vector<Triplet>& trip, Batch
 inline void shard_range(const BatchPlan& B, int shard, int nshards, size_t& b0, size_t& b1) {
     const size_t nbatch = B.bstart.size() - 1;
     const long long njobs = (long long)B.jobs.size();
-    auto cut = [&](int s) -> size_t {      // first batch whose jobs start at or after the s-th equal share
+    auto cut = [&](int s) -> size_t {      // the batch boundary nearest to the s-th equal share of the jobs
         if (s <= 0) return 0;
         if (s >= nshards) return nbatch;
         const long long target = njobs * s / nshards;
         size_t b = 0;
         while (b < nbatch && B.jstart[b] < target) ++b;
+        if (b > 0 && target - B.jstart[b - 1] < B.jstart[b] - target) --b;
         return b;
     };
     b0 = cut(shard);

@@ -130,23 +130,27 @@ __device__ __forceinline__ void pack_split_store(uint32_t* __restrict__ row, flo
 }
 
 // Source viewed as [d][s], s = bc * ro + r (resident vvvo: ro = o, the slice of r goes to slot r) or s = bc
-// (one streamed slice (ab|c r): ro = 1, slot0 = its slot).  One CTA moves a (32 d) x (PKX_SPAN s) brick through
-// shared memory and writes whole 128-byte packed rows; blockIdx.y = K chunk.
+// (one FP64 slice (db|c r): ro = 1, slot0 = its slot); sp = c-pitch of the source (v, or vp for a slice the RI
+// builder wrote).  One CTA moves a (32 d) x (PKX_SPAN s) brick through shared memory and writes whole 128-byte
+// packed rows; blockIdx.y = K chunk.
 constexpr int PKX_SPAN = 256;
 constexpr int PKX_PITCH = PKX_SPAN + 1;
 constexpr int PKX_SMEM = 32 * PKX_PITCH * 8;
 __global__ void __launch_bounds__(256)
-pack_xk_kernel(const double* __restrict__ src, int v, int vp, int vk, int ro, int slot0, uint32_t* __restrict__ XK,
-               uint32_t* __restrict__ XKT, const float* __restrict__ scale_ptr) {
+pack_xk_kernel(const double* __restrict__ src, int v, int vp, int vk, int ro, int sp, int slot0,
+               uint32_t* __restrict__ XK, uint32_t* __restrict__ XKT, const float* __restrict__ scale_ptr) {
     const double scale = (double)*scale_ptr;
     extern __shared__ double tile[];                 // [32][PKX_PITCH]
     const int d0 = blockIdx.y * 32;
     const size_t S = (size_t)v * v * ro;
     const size_t s0 = (size_t)blockIdx.x * PKX_SPAN;
     const int cnt = (int)min((size_t)PKX_SPAN, S - s0);
+    const size_t Sd = (size_t)v * sp * ro;           // source elements per d
     for (int e = threadIdx.x; e < 32 * cnt; e += 256) {
         const int dd = e / cnt, s = e % cnt;
-        tile[dd * PKX_PITCH + s] = d0 + dd < v ? src[(size_t)(d0 + dd) * S + s0 + s] : 0.0;
+        size_t off = s0 + s;
+        if (sp != v) { const size_t bc = off / ro; off = ((bc / v) * sp + bc % v) * ro + off % ro; }
+        tile[dd * PKX_PITCH + s] = d0 + dd < v ? src[(size_t)(d0 + dd) * Sd + off] : 0.0;
     }
     __syncthreads();
     const size_t plane = (size_t)v * vp * vk;        // words of one slot

@@ -325,11 +325,11 @@ int transpose_slice(const Plan& P, const double* X, double* XT, cudaStream_t st)
 }
 
 // src viewed as [d][s]: the resident vvvo (ro = o, slot = r) or one FP64 slice (ro = 1) -> packed XK / XKT slots
-int pack_xk(const Plan& P, const double* src, int ro, int slot0, const Operands& op, cudaStream_t st) {
+int pack_xk(const Plan& P, const double* src, int ro, int sp, int slot0, const Operands& op, cudaStream_t st) {
     CU_TRY(cudaFuncSetAttribute(pack_xk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PKX_SMEM));
     const size_t S = (size_t)P.v * P.v * ro;
     dim3 grid((unsigned)((S + PKX_SPAN - 1) / PKX_SPAN), P.vk / 32);
-    pack_xk_kernel<<<grid, 256, PKX_SMEM, st>>>(src, P.v, P.vp, P.vk, ro, slot0, (uint32_t*)op.x, (uint32_t*)op.xt,
+    pack_xk_kernel<<<grid, 256, PKX_SMEM, st>>>(src, P.v, P.vp, P.vk, ro, sp, slot0, (uint32_t*)op.x, (uint32_t*)op.xt,
                                                 op.scales);
     CU_TRY(cudaGetLastError());
     ++g_launches;
@@ -412,7 +412,7 @@ int run_prepare(const Plan& P, const Inputs& in, const Source& src, const Operan
         g_launches += 3;
     }
     if (src.mode == SLICES_RESIDENT)
-        if (int rc = pack_xk(P, src.vvvo, o, 0, op, st)) return rc;
+        if (int rc = pack_xk(P, src.vvvo, o, v, 0, op, st)) return rc;
     {
         dim3 grid(o * v, (v + 63) / 64, (o + 63) / 64);
         pack_t2k_kernel<<<grid, 256, 0, st>>>(in.t2, v, P.vp, o, P.ok, (uint32_t*)op.t2k, (uint32_t*)op.t2kt, op.scales + 1);
@@ -592,7 +592,7 @@ int run_batches(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws,
                 } else {   // one FP64 staging slice: build, split-pack, next
                     for (int l = l0; l < l1; ++l) {
                         if (int rc = launch_ri(P, maps, d_loads + B.loads.size() + l, 1, op.stage, st)) return rc;
-                        if (int rc = pack_xk(P, op.stage, 1, B.loads[l].slot, op, st)) return rc;
+                        if (int rc = pack_xk(P, op.stage, 1, P.vp, B.loads[l].slot, op, st)) return rc;
                     }
                 }
             }
@@ -602,7 +602,7 @@ int run_batches(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws,
                     if (int rc = transpose_slice(P, (const double*)op.x + (size_t)ld.slot * P.n_slice,
                                                  (double*)op.xt + (size_t)ld.slot * P.n_slice, st)) return rc;
                 } else if (streamed) {
-                    if (int rc = pack_xk(P, stage_of(b, l - l0), 1, ld.slot, op, st)) return rc;
+                    if (int rc = pack_xk(P, stage_of(b, l - l0), 1, v, ld.slot, op, st)) return rc;
                 }
             }
         }
@@ -725,8 +725,8 @@ bool fit_plan(int o, int v, int prec, int mode, int naux, size_t bytes, Plan& P)
         if (!make_plan(o, v, prec, M, mode, 0, naux, win)) return false;
         if (M.win < win) continue;                 // capped already (U budget or o): same plan as a smaller cap
         if (M.total > bytes) continue;
-        const size_t per_slot = 2 * align_up(M.n_slice * M.esz, 1024);
-        long long n = M.nslots + (long long)((bytes - M.total) / per_slot);
+        const size_t per_slot = 2 * M.n_slice * M.esz;          // before alignment: an upper estimate, walked down
+        long long n = M.nslots + (long long)((bytes - M.total) / per_slot) + 1;
         if (n > o) n = o;
         for (; n >= M.nslots; --n)
             if (make_plan(o, v, prec, P, mode, (int)n, naux, win) && P.total <= bytes) return true;

@@ -107,11 +107,17 @@ def make_inputs_device(nocc: int, nvirt: int, naux: int, seed: int = 0, t1_sigma
     Boo = Bd[:, :o, :o].reshape(naux, o * o)
     Bov = Bd[:, :o, o:].reshape(naux, o * v)
     Bvo = Bd[:, o:, :o].reshape(naux, v * o).contiguous()
+    # (ab|ck) = (ba|ck): only the blocks b >= a0 of every a-chunk go through the GEMM (half the generator's flops,
+    # which at configs[4] are 1.3e16 in FP64); the rest is their mirror image
     vvvo = torch.empty((v, v, v, o), dtype=torch.float64, device=device)
     for a0 in range(0, v, chunk):
         a1 = min(v, a0 + chunk)
-        Bvv = Bd[:, o + a0:o + a1, o:].reshape(naux, (a1 - a0) * v)
-        vvvo[a0:a1] = (Bvv.T @ Bvo).reshape(a1 - a0, v, v, o)
+        Bvv = Bd[:, o + a0:o + a1, o + a0:].reshape(naux, (a1 - a0) * (v - a0))
+        blk = (Bvv.T @ Bvo).reshape(a1 - a0, v - a0, v, o)
+        vvvo[a0:a1, a0:] = blk
+        if a1 < v:
+            vvvo[a1:, a0:a1] = blk[:, a1 - a0:].permute(1, 0, 2, 3)
+        del blk
     ovoo = (Bov.T @ Boo).reshape(o, v, o, o).contiguous()
     ovov = (Bov.T @ Bov).reshape(o, v, o, v).contiguous()
     eo = torch.from_numpy(eps_o).to(device)

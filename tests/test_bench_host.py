@@ -28,7 +28,16 @@ import bench
 dist.init_process_group("gloo")
 rank = dist.get_rank()
 t, u = bench.reduce_over_ranks(1.0 + rank, 10.0 * (rank + 1), dist.get_world_size())
-print(json.dumps({{"rank": rank, "t": t, "u": u}}), flush=True)
+# triplet-sharded mode: every rank holds its shard's partial (E(T), E[4], E[5]); the ordered sum is the total
+import paper_1609_08094_b200 as tb
+o, v = 9, 40
+_, sot, jps = tb.triples_plan_shards(o, v, tb.FP64, dist.get_world_size())
+fake = [1e-3 * (n + 1) * (1 + 1e-7 * n) for n in range(len(sot))]          # a stand-in energy per triplet
+mine = sum(fake[n] for n in range(len(sot)) if sot[n] == rank)
+tot = bench.combine_shard_partials((mine, mine, 0.0), dist.get_world_size())
+print(json.dumps({{"rank": rank, "t": t, "u": u, "tot": tot, "mine": mine, "covered": int((sot == rank).sum()),
+                  "all": int((sot >= 0).sum()), "jobs": [int(x) for x in jps],
+                  "single": sum(fake[n] for n in range(len(sot)) if sot[n] >= 0)}}), flush=True)
 dist.destroy_process_group()
 """
 
@@ -49,6 +58,14 @@ def test_reduce_over_ranks_world_size_2_gloo():
         outs.append(json.loads(out.strip().splitlines()[-1]))
     for o in outs:
         assert o["t"] == 2.0 and o["u"] == 30.0       # max(1, 2) seconds, 10 + 20 units on every rank
+    # sharded mode: the two ranks cover every non-diagonal triplet exactly once, both ranks get
+    # the same rank-ordered total, and it equals the single-rank sum to rounding
+    assert outs[0]["covered"] + outs[1]["covered"] == outs[0]["all"] and min(o["covered"] for o in outs) > 0
+    assert outs[0]["tot"] == outs[1]["tot"]
+    by_rank = sorted(outs, key=lambda o: o["rank"])
+    assert outs[0]["tot"][0] == by_rank[0]["mine"] + by_rank[1]["mine"]
+    assert abs(outs[0]["tot"][0] - outs[0]["single"]) <= 1e-13 * abs(outs[0]["single"])
+    assert max(outs[0]["jobs"]) <= 1.6 * min(outs[0]["jobs"])          # whole window blocks, near-equal task weight (L198)
 
 
 def test_reduce_over_ranks_single_process_is_identity():
@@ -82,7 +99,7 @@ def test_reference_arm_times_the_oracle_and_prints_one_json_line():
     assert len(lines) == 1
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["unit"] == "TFLOP/s" and d["higher_is_better"] is True
-    assert d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
+    assert d["value"] > 0 and d["cpu_baseline"]["kind"].startswith("oracle") and d["cpu_baseline"]["cores"] >= 1
     assert d["e2e"] == {"value": d["value"], "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert d["gpu_launches"] == 0 and "tiny" in d["config"]["workload"]
 
