@@ -164,3 +164,90 @@ def test_fp64_peak_probe():
     ws = ws_bytes(1 << 20)
     tf = tb.triples_probe_fp64_peak(ws, iters=4000)
     assert 20.0 < tf < 60.0, tf           # B200: 148 SM x 128 flop/clk x ~1.9 GHz = ~37 TFLOP/s
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# BASELINE.json configs at full size through the NEXT-1 / NEXT-2 entry points, against the stored oracle values
+# ------------------------------------------------------------------------------------------------------------------
+def _golden(name):
+    import json
+    import os
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name + ".json")) as f:
+        return json.load(f)
+
+
+def _check_against_golden(g, et, o, tol):
+    index = {t: n for n, t in enumerate(synth.triplet_list(o))}
+    want = np.array(g["energies"])
+    n_cmp = 0
+    for n, t in enumerate(g["triplets_ijk"]):
+        if t[0] == t[1] == t[2]:
+            continue
+        got = et[index[tuple(t)]]
+        assert abs(got[0] - want[n, 0]) <= tol * abs(want[n, 1]) and abs(got[1] - want[n, 1]) <= tol * abs(want[n, 1]), (t, got, want[n])
+        n_cmp += 1
+    return n_cmp
+
+
+def test_medium_streamed_with_a_budget_below_vvvo_is_bitwise_the_resident_run():
+    """configs[2] (vvvo 2.65 GB) with a device workspace SMALLER than the vvvo tensor: window 1, six cache slots,
+    2576 batches, ~3000 slice loads.  Per-triplet energies bitwise equal to the resident run, and within 1e-10 of
+    the oracle's stored values."""
+    o, v, naux = synth.CONFIGS["medium"]
+    d = synth.make_inputs_device(o, v, naux, seed=0)
+    args = [d[k] for k in ("eps_o", "eps_v", "t1", "t2", "vvvo", "ovoo", "ovov")]
+    T = tb.triples_triplet_count(o)
+    et = torch.zeros((T, 3), dtype=torch.float64, device="cuda")
+    ws = ws_bytes(tb.triples_workspace_bytes(o, v, tb.FP64))
+    E = tb.triples_energy(o, v, *args, tb.FP64, ws, e_triplet_out=et)
+    del ws
+    host = torch.empty((o, v, v, v), dtype=torch.float64, pin_memory=True)
+    for k in range(o):
+        host[k].copy_(d["vvvo"][:, :, :, k])
+    torch.cuda.synchronize()
+    nbytes = tb.triples_workspace_bytes_streamed(o, v, tb.FP64, 0, 1)
+    assert nbytes < 8 * v ** 3 * o, "the budget must be smaller than the tensor that is streamed"
+    assert tb.triples_cache_slots(o, v, 0, tb.FP64, STREAMED, nbytes) == (6, 1)
+    ets = torch.zeros_like(et)
+    Es = tb.triples_energy_streamed(o, v, d["eps_o"], d["eps_v"], d["t1"], d["t2"], host.numpy(), d["ovoo"], d["ovov"],
+                                    tb.FP64, ws_bytes(nbytes), e_triplet_out=ets)
+    assert Es == E and torch.equal(ets, et)
+    g = _golden("medium_full")
+    assert _check_against_golden(g, ets.cpu().numpy(), o, 1e-10) >= 64
+
+
+@pytest.mark.parametrize("name,prec", [("small", tb.FP64), ("small", tb.MIXED), ("medium", tb.FP64)],
+                         ids=["small-fp64", "small-mixed", "medium-fp64"])
+def test_ri_direct_at_config_size_against_oracle_goldens(name, prec):
+    """configs[1..2] without a vvvo tensor on the device: every stored triplet of the oracle's full goldens."""
+    o, v, naux = synth.CONFIGS[name]
+    eps_o, eps_v, t1, t2, ovoo, ovov, B = synth.make_inputs_sliced(o, v, naux, seed=0)
+    dv = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (eps_o, eps_v, t1, t2, B, ovoo, ovov)]
+    T = tb.triples_triplet_count(o)
+    et = torch.zeros((T, 3), dtype=torch.float64, device="cuda")
+    nbytes = tb.triples_workspace_bytes_ri(o, v, naux, prec, o // 2, 0)          # half the slices cached: rebuilds happen
+    E = tb.triples_energy_ri(o, v, naux, *dv, prec, ws_bytes(nbytes), e_triplet_out=et)
+    g = _golden(name + "_full")
+    tol = TOL[prec]
+    n_cmp = _check_against_golden(g, et.cpu().numpy(), o, tol)
+    assert n_cmp >= 64
+    if g["complete"]:
+        assert abs(E[0] - g["E"][0]) <= tol * abs(g["E"][0]) and abs(E[1] - g["E"][1]) <= tol * abs(g["E"][1])
+
+
+def test_mixed_run_is_bitwise_repeatable_on_a_ragged_size():
+    """Stress of the CTA-pair hand-offs of the mixed contraction (TMA of both CTAs on the leader's barrier, relaxed
+    remote arrives for the TMEM buffers): 25 repeats of a ragged-size run must agree bit for bit."""
+    inp = synth.make_inputs(7, 75, 40, seed=13, t1_sigma=0.1)
+    o, v = inp.nocc, inp.nvirt
+    d = dev(inp)
+    ws = ws_bytes(tb.triples_workspace_bytes(o, v, tb.MIXED))
+    T = tb.triples_triplet_count(o)
+    ref = None
+    for _ in range(25):
+        et = torch.zeros((T, 3), dtype=torch.float64, device="cuda")
+        E = tb.triples_energy(o, v, *d, tb.MIXED, ws, e_triplet_out=et)
+        if ref is None:
+            ref = (E, et.clone())
+        else:
+            assert E == ref[0] and torch.equal(et, ref[1])
