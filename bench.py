@@ -39,6 +39,7 @@ if ROOT not in sys.path:
 
 NAMES = ("eps_o", "eps_v", "t1", "t2", "vvvo", "ovoo", "ovov")
 MIXED_DTYPE = "fp16 split x = h + l (f32 accumulate), f64 reduction"
+EMU_DTYPE = "f64 emulated: 7 base-128 int8 digits per operand, 28 exact s8 x s8 -> s32 products, f64 recombination and reduction"
 GOLDEN_OF = {"small": "small_full", "medium": "medium_full", "large": "large_sample", "largest": "largest_sample"}
 
 
@@ -249,6 +250,13 @@ def rooflines(tb, prec, prof, peaks, peak_kind, fp64_peak, traffic):
         kernel = "gemm_f64_kernel"
         peak = fp64_peak["tflops"]
         peak_note = fp64_peak["note"]
+    elif prec == tb.EMU64:
+        kernel = "gemm_emu64_kernel"
+        peak = peaks["bf16_tflops_sustained"] * 2.0 / 28.0
+        peak_note = (f"INT8 dense tensor rate = 2 x bf16 sustained cuBLAS ({peak_kind}, MEASURED_PEAKS.json; the guide's nominal "
+                     "int8:bf16 ratio) / 28: every FP64-class product costs 28 int8 digit products (levels <= 6 of 7 x 7 "
+                     "digits). achieved = ALGORITHMIC flops; vs_native_fp64_peak = achieved / the DMMA peak measured in "
+                     "this run (> 1: faster than the native FP64 tensor pipe can go)")
     else:
         kernel = "gemm_f16split_kernel"
         peak = peaks["bf16_tflops_sustained"] * 0.5
@@ -260,11 +268,14 @@ def rooflines(tb, prec, prof, peaks, peak_kind, fp64_peak, traffic):
             "frac": gemm_tflops / peak, "traffic": None, "peak_note": peak_note,
             "share_of_step": prof["contraction_ms"] / step_ms, "launches_per_step": prof["contraction_launches"],
             "flops_per_launch": prof["contraction_flops"] / nl, "avg_launch_ms": prof["contraction_ms"] / nl}
-    if prec != tb.FP64:
+    if prec == tb.MIXED:
         roof["tensor_pipe_tf32_equiv"] = 1.5 * gemm_tflops
         roof["frac_tensor_pipe"] = 1.5 * gemm_tflops / peak
+    if prec == tb.EMU64:
+        roof["tensor_pipe_int8"] = 28.0 * gemm_tflops
+        roof["vs_native_fp64_peak"] = gemm_tflops / fp64_peak["tflops"]
     nr = max(prof["reduction_launches"], 1)
-    red = {"bound": "hbm", "kernel": "reduce_kernel<double>" if prec == tb.FP64 else "reduce_kernel<float>",
+    red = {"bound": "hbm", "kernel": "reduce_kernel<float>" if prec == tb.MIXED else "reduce_kernel<double>",
            "achieved": red_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": red_gbs / peaks["hbm_gbs"],
            "traffic": None,
            "peak_note": f"{peak_kind} copy bandwidth (read + write); the reduction only reads, and a pure read stream "
@@ -323,13 +334,17 @@ def precision_leg(tb, torch, config, prec, o, v, dargs, ws, stream, steps, warmu
     clocks = sampler.stop()
     prof = profiled_step(tb, lambda: tb.triples_energy(o, v, *dargs, prec, ws, stream=stream))
     roof, red = rooflines(tb, prec, prof, peaks, peak_kind, fp64_peak, load_traffic(config))
-    tol = 1e-10 if prec == tb.FP64 else 1e-5
+    tol = 1e-5 if prec == tb.MIXED else 1e-10
     leg = {"value": formula_flops(o, v) / sec / 1e12, "executed_value": prof["contraction_flops"] / sec / 1e12,
            "unit": "TFLOP/s", "s_per_ET": sec, "steps": steps, "warmup": warmup,
-           "dtype": "f64" if prec == tb.FP64 else MIXED_DTYPE, "E_T": E[0], "E4": E[1], "E5": E[2],
+           "dtype": dtype_name(tb, prec), "E_T": E[0], "E4": E[1], "E5": E[2],
            "roofline": roof, "roofline_reduction": red, "clocks": clocks,
            "parity": parity_vs_golden(config, et.cpu().numpy(), index, tol)}
     return leg, E
+
+
+def dtype_name(tb, prec):
+    return "f64" if prec == tb.FP64 else (MIXED_DTYPE if prec == tb.MIXED else EMU_DTYPE)
 
 
 def streamed_leg(tb, torch, o, v, d, prec, stream, nslots, win, resident_sec, E_resident):
@@ -369,7 +384,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", default="medium", choices=["tiny", "small", "medium", "large", "largest"])
-    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"])
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed", "emu64"])
     ap.add_argument("--ref-triplets", type=int, default=2, help="triplets per step of the reference arm")
     ap.add_argument("--cpu-triplets", type=int, default=4, help="triplets of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -402,8 +417,8 @@ def main():
 
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    prec = tb.FP64 if args.precision == "fp64" else tb.MIXED
-    tol = 1e-10 if prec == tb.FP64 else 1e-5
+    prec = {"fp64": tb.FP64, "mixed": tb.MIXED, "emu64": tb.EMU64}[args.precision]
+    tol = 1e-5 if prec == tb.MIXED else 1e-10
     o, v, naux = synth.CONFIGS[args.config]
     default_line = args.config == "medium" and prec == tb.FP64 and world == 1
     # ---- synthetic inputs: host copies (pinned, for the e2e leg and the oracle) and device-resident copies
@@ -424,7 +439,7 @@ def main():
     mixed_leg = prec == tb.FP64 and world == 1 and not args.no_mixed_leg and args.config in ("tiny", "small", "medium")
     ws_bytes = tb.triples_workspace_bytes_host(o, v, prec)
     if mixed_leg:
-        ws_bytes = max(ws_bytes, tb.triples_workspace_bytes(o, v, tb.MIXED))
+        ws_bytes = max(ws_bytes, tb.triples_workspace_bytes(o, v, tb.MIXED), tb.triples_workspace_bytes(o, v, tb.EMU64))
     ws = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
     T = tb.triples_triplet_count(o)
@@ -596,7 +611,7 @@ def main():
             "metric": "(T) TFLOP/s", "value": value, "executed_value": executed_value, "unit": "TFLOP/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "s_per_ET": ms_per_step / 1e3,
             "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
-            "dtype": "f64" if prec == tb.FP64 else MIXED_DTYPE, "data": "synthetic",
+            "dtype": dtype_name(tb, prec), "data": "synthetic",
             "config": {"workload": workload_name(args.config, args.precision, o, v, naux),
                        "parallelism": (f"triplet-sharded x{world}" if sharded else f"replicas x{world}"),
                        "l2": f"inputs larger than L2 (vvvo {8*v**3*o/1e6:.0f} MB, U buffers re-written every batch)",

@@ -5,6 +5,7 @@ its thin Python binding (``binding``) plus the seeded synthetic-input generator 
 tests and the benchmark.  There is no CPU fallback: the binding raises if the CUDA library is missing.
 """
 from .binding import (  # noqa: F401
+    EMU64,
     FP64,
     MIXED,
     TriplesError,

@@ -12,6 +12,7 @@ import numpy as np
 
 FP64 = 0
 MIXED = 1
+EMU64 = 2
 
 _STATUS = {0: "OK", 1: "EINVAL", 2: "EWORKSPACE", 3: "ECUDA", 4: "EARCH"}
 _HERE = os.path.dirname(os.path.abspath(__file__))

@@ -86,7 +86,9 @@ struct Plan {
     int red_gx = 0;             // CTA columns of the fused reduction (orbit stride), fixed by v
     size_t n_side = 0;          // doubles of one triplet's side buffer (reduce.cuh)
     size_t off_side = 0;
-    size_t esz = 8;             // bytes per stored operand / U element
+    size_t esz = 8;             // bytes per stored U element (FP64 / emulated FP64: 8, mixed: 4)
+    size_t osz = 8;             // bytes per stored operand word (FP64: 8; mixed and emulated FP64: 4-byte packed words)
+    int kwords = 32;            // packed paths: 4-byte words per operand row and 32-wide K chunk (mixed 32, emulated 64)
     size_t n_x = 0, n_ot = 0, n_t2 = 0, n_u = 0;   // elements of one X (or XT), Ot, T2, one U buffer
     size_t n_t2k = 0;                              // mixed: elements of T2K (or T2KT)
     size_t off_t2k = 0, off_t2kt = 0;
@@ -115,13 +117,16 @@ inline int min_slots(int o, int win, int mode) {
 // needs fewer U buffers and a smaller minimum cache: how a streamed / RI run fits a small device budget).
 inline bool make_plan(int o, int v, int prec, Plan& P, int mode = SLICES_RESIDENT, int nslots = 0, int naux = 0,
                       int win_cap = 0) {
-    if (o < 1 || v < 1 || o > kMaxOcc || v > kMaxVirt || (prec != 0 && prec != 1)) return false;
+    if (o < 1 || v < 1 || o > kMaxOcc || v > kMaxVirt || (prec < 0 || prec > 2)) return false;
+    if (prec == 2 && mode != SLICES_RESIDENT) return false;     // emulated FP64: resident slices only
     if (mode < 0 || mode > 2 || nslots < 0 || (mode == SLICES_RI && naux < 1)) return false;
     P = Plan();
     P.o = o; P.v = v; P.prec = prec; P.mode = mode;
     P.vp = (v + 1) & ~1;
     P.op = (o + 1) & ~1;
-    P.esz = prec == 0 ? 8 : 4;
+    P.esz = prec == 1 ? 4 : 8;
+    P.osz = prec == 0 ? 8 : 4;
+    P.kwords = prec == 2 ? 64 : 32;
     P.T = triplet_count(o);
     P.norb = (int)orbit_count(v);
     // CTA tile: the M tile (40, 80 or 120 rows) that wastes the fewest padded rows; ties -> larger tile
@@ -142,11 +147,11 @@ inline bool make_plan(int o, int v, int prec, Plan& P, int mode = SLICES_RESIDEN
     P.nt = num_red_tiles(v);
     P.n_u = (size_t)P.nt * P.nt * P.nt * 512;          // blocked layout of ulayout.cuh
     P.n_side = (size_t)P.nt * P.nt * 448;             // tile-pair records of reduce.cuh
-    if (prec == 1) {   // packed K-major operands, transposed tiles (gemm_f16split.cuh)
-        P.vk = (v + 31) & ~31;     // whole 32-wide K chunks (one 128-byte packed row each)
-        P.ok = (o + 31) & ~31;
-        P.tf_ntiles = (v + 255) / 256;
-        P.tf_bn = (((v + P.tf_ntiles - 1) / P.tf_ntiles) + 15) & ~15;
+    if (prec != 0) {   // packed K-major operands, transposed tiles (gemm_f16split.cuh / gemm_emu64.cuh)
+        P.vk = ((v + 31) / 32) * P.kwords;     // whole 32-wide K chunks (one / two 128-byte packed rows each)
+        P.ok = ((o + 31) / 32) * P.kwords;
+        P.tf_ntiles = prec == 1 ? (v + 255) / 256 : (v + 63) / 64;
+        P.tf_bn = prec == 1 ? ((((v + P.tf_ntiles - 1) / P.tf_ntiles) + 15) & ~15) : 64;
         P.tf_mtiles = (int)((N + 127) / 128);
         // CTA pairs (cta_group::2): a pair owns two consecutive m-tiles, each CTA stages half of the N-side rows
         // (tf_bn is a multiple of 16, so a half is whole 8-row swizzle atoms)
@@ -192,13 +197,13 @@ inline bool make_plan(int o, int v, int prec, Plan& P, int mode = SLICES_RESIDEN
 
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t at = off; off = align_up(off + bytes, 1024); return at; };
-    P.off_x = take(P.n_x * P.esz);
-    P.off_xt = take(P.n_x * P.esz);
-    P.off_ot = take(P.n_ot * P.esz);
-    P.off_t2 = take(P.n_t2 * P.esz);
-    if (prec == 1) {   // occupied-segment M-side operands of the transposed mixed GEMM
-        P.off_t2k = take(P.n_t2k * P.esz);
-        P.off_t2kt = take(P.n_t2k * P.esz);
+    P.off_x = take(P.n_x * P.osz);
+    P.off_xt = take(P.n_x * P.osz);
+    P.off_ot = take(P.n_ot * P.osz);
+    P.off_t2 = take(P.n_t2 * P.osz);
+    if (prec != 0) {   // occupied-segment M-side operands of the transposed GEMMs
+        P.off_t2k = take(P.n_t2k * P.osz);
+        P.off_t2kt = take(P.n_t2k * P.osz);
     }
     if (P.nstage) P.off_stage = take((size_t)P.nstage * v * v * P.vp * 8);
     if (mode == SLICES_RI) {

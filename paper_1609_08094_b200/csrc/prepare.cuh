@@ -40,6 +40,8 @@ __global__ void scales_kernel(const unsigned int* __restrict__ maxbits, float* _
     scales[0] = ldexpf(1.0f, s[0]);
     scales[1] = ldexpf(1.0f, s[1]);
     scales[2] = ldexpf(1.0f, -(s[0] + s[1]));
+    reinterpret_cast<int*>(scales)[12] = s[0];       // the exponents themselves (emulated-FP64 path, gemm_emu64.cuh)
+    reinterpret_cast<int*>(scales)[13] = s[1];
 }
 
 // vvvo viewed as [R = v^3][o]: each CTA moves RB consecutive rows (one contiguous span) through smem.
@@ -129,6 +131,40 @@ __device__ __forceinline__ void pack_split_store(uint32_t* __restrict__ row, flo
     row[(lane >> 1) + (odd ? 16 : 0)] = odd ? (got | (mine << 16)) : (mine | (got << 16));
 }
 
+// Emulated-FP64 path (gemm_emu64.cuh): the scaled value is rounded to a 49-bit fixed-point integer
+// xi = rint(x * 2^(s + 33)) (|xi| < 2^47: the class maximum sits in [2^46, 2^47)) and cut into seven balanced base-128
+// digits d_0 (most significant) .. d_6 in [-64, 63], xi = sum_i d_i 128^(6-i).  Per operand row and 32-wide K chunk TWO
+// 128-byte rows: bytes [32 i, 32 i + 32) of the first hold digit i = 0..3 of the 32 K elements, of the second digit
+// i = 4..6 (the last 32 bytes are zero).  The 32 lanes of a warp hold 32 consecutive K elements.
+constexpr int EMU_SHIFT = 33;
+__device__ __forceinline__ void pack_emu_store(uint32_t* __restrict__ row2, double x, int lane) {
+    long long xi = __double2ll_rn(x);
+    int8_t d[8];
+#pragma unroll
+    for (int i = 6; i >= 0; --i) {
+        int r = (int)(xi & 127);
+        if (r >= 64) r -= 128;
+        d[i] = (int8_t)r;
+        xi = (xi - r) >> 7;
+    }
+    d[7] = 0;
+    int8_t* b = reinterpret_cast<int8_t*>(row2);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) b[(i >> 2) * 128 + (i & 3) * 32 + lane] = d[i];
+}
+// one packed K chunk of one operand row: MODE 0 = FP16 split (32 words), MODE 1 = emulated FP64 digits (64 words)
+template <int MODE>
+__device__ __forceinline__ void pack_store(uint32_t* __restrict__ row, double x, double scale, int lane) {
+    if constexpr (MODE == 0) pack_split_store(row, (float)(x * scale), lane);
+    else pack_emu_store(row, x * scale, lane);
+}
+// scale of a tensor class: sc = the scales block of prepare (floats 2^sg, 2^st, .. ; ints sg, st at [12], [13])
+template <int MODE>
+__device__ __forceinline__ double pack_scale(const float* __restrict__ sc, int cls) {
+    if constexpr (MODE == 0) return (double)sc[cls];
+    else return ldexp(1.0, reinterpret_cast<const int*>(sc)[12 + cls] + EMU_SHIFT);
+}
+
 // Source viewed as [d][s], s = bc * ro + r (resident vvvo: ro = o, the slice of r goes to slot r) or s = bc
 // (one FP64 slice (db|c r): ro = 1, slot0 = its slot); sp = c-pitch of the source (v, or vp for a slice the RI
 // builder wrote).  One CTA moves a (32 d) x (PKX_SPAN s) brick through shared memory and writes whole 128-byte
@@ -136,10 +172,12 @@ __device__ __forceinline__ void pack_split_store(uint32_t* __restrict__ row, flo
 constexpr int PKX_SPAN = 256;
 constexpr int PKX_PITCH = PKX_SPAN + 1;
 constexpr int PKX_SMEM = 32 * PKX_PITCH * 8;
+template <int MODE>
 __global__ void __launch_bounds__(256)
 pack_xk_kernel(const double* __restrict__ src, int v, int vp, int vk, int ro, int sp, int slot0,
-               uint32_t* __restrict__ XK, uint32_t* __restrict__ XKT, const float* __restrict__ scale_ptr) {
-    const double scale = (double)*scale_ptr;
+               uint32_t* __restrict__ XK, uint32_t* __restrict__ XKT, const float* __restrict__ sc) {
+    constexpr int CW = MODE ? 64 : 32;               // words per K chunk
+    const double scale = pack_scale<MODE>(sc, 0);
     extern __shared__ double tile[];                 // [32][PKX_PITCH]
     const int d0 = blockIdx.y * 32;
     const size_t S = (size_t)v * v * ro;
@@ -161,19 +199,21 @@ pack_xk_kernel(const double* __restrict__ src, int v, int vp, int vk, int ro, in
         const int r = (int)(sg % ro);
         const size_t bc = sg / ro;
         const int b = (int)(bc / v), c = (int)(bc % v);
-        const float xs = (float)(tile[lane * PKX_PITCH + s] * scale);
-        const size_t base = (size_t)(slot0 + r) * plane + d0;
-        pack_split_store(XK + base + ((size_t)b * vp + c) * vk, xs, lane);
-        pack_split_store(XKT + base + ((size_t)c * vp + b) * vk, xs, lane);
+        const double x = tile[lane * PKX_PITCH + s];
+        const size_t base = (size_t)(slot0 + r) * plane + (size_t)blockIdx.y * CW;
+        pack_store<MODE>(XK + base + ((size_t)b * vp + c) * vk, x, scale, lane);
+        pack_store<MODE>(XKT + base + ((size_t)c * vp + b) * vk, x, scale, lane);
     }
 }
 
 // blockIdx.x = q*v + x (x = b for T2K, x = c for T2KT), blockIdx.y = chunk of 64 along the contiguous source index y,
 // blockIdx.z = chunk of 64 along l (two packed rows).
+template <int MODE>
 __global__ void __launch_bounds__(256)
 pack_t2k_kernel(const double* __restrict__ t2, int v, int vp, int o, int ok, uint32_t* __restrict__ T2K,
-                uint32_t* __restrict__ T2KT, const float* __restrict__ scale_ptr) {
-    const double scale = (double)*scale_ptr;
+                uint32_t* __restrict__ T2KT, const float* __restrict__ sc) {
+    constexpr int CW = MODE ? 64 : 32;
+    const double scale = pack_scale<MODE>(sc, 1);
     __shared__ double tile[64][65];
     const int q = blockIdx.x / v, x = blockIdx.x % v;
     const int y0 = blockIdx.y * 64, l0 = blockIdx.z * 64;
@@ -186,42 +226,46 @@ pack_t2k_kernel(const double* __restrict__ t2, int v, int vp, int o, int ok, uin
     const int lane = threadIdx.x & 31;
     for (int e = threadIdx.x; e < 64 * ny; e += 256) {       // a warp = 32 consecutive l of one y
         const int lh = (e >> 5) & 1, yy = e >> 6;
-        if (l0 + lh * 32 >= ok) continue;                    // warp-uniform
-        const float xs = (float)(tile[lh * 32 + lane][yy] * scale);
-        const int l = l0 + lh * 32;
-        pack_split_store(T2K + (((size_t)q * v + x) * vp + (y0 + yy)) * ok + l, xs, lane);     // T2K [q][b=x][c=y][l]
-        pack_split_store(T2KT + (((size_t)q * v + (y0 + yy)) * vp + x) * ok + l, xs, lane);    // T2KT[q][b=y][c=x][l]
+        const int l = (l0 / 32 + lh) * CW;                   // word offset of this K chunk in a row
+        if (l >= ok) continue;                               // warp-uniform
+        const double xv = tile[lh * 32 + lane][yy];
+        pack_store<MODE>(T2K + (((size_t)q * v + x) * vp + (y0 + yy)) * ok + l, xv, scale, lane);     // T2K [q][b=x][c=y][l]
+        pack_store<MODE>(T2KT + (((size_t)q * v + (y0 + yy)) * vp + x) * ok + l, xv, scale, lane);    // T2KT[q][b=y][c=x][l]
     }
 }
 
 // T2A[row][d], row = (p,q,a): one warp per (row, K chunk)
+template <int MODE>
 __global__ void __launch_bounds__(256)
 pack_t2a_kernel(const double* __restrict__ t2, size_t rows, int v, int vk, uint32_t* __restrict__ T2A,
-                const float* __restrict__ scale_ptr) {
-    const double scale = (double)*scale_ptr;
-    const int lane = threadIdx.x & 31, nch = vk / 32;
+                const float* __restrict__ sc) {
+    constexpr int CW = MODE ? 64 : 32;
+    const double scale = pack_scale<MODE>(sc, 1);
+    const int lane = threadIdx.x & 31, nch = vk / CW;
     const size_t nw = rows * nch;
     for (size_t w = blockIdx.x * (size_t)8 + (threadIdx.x >> 5); w < nw; w += (size_t)gridDim.x * 8) {
         const size_t row = w / nch;
-        const int d = (int)(w % nch) * 32 + lane;
-        const float xs = d < v ? (float)(t2[row * v + d] * scale) : 0.0f;
-        pack_split_store(T2A + row * vk + (d - lane), xs, lane);
+        const int ch = (int)(w % nch), d = ch * 32 + lane;
+        const double x = d < v ? t2[row * v + d] : 0.0;
+        pack_store<MODE>(T2A + row * vk + (size_t)ch * CW, x, scale, lane);
     }
 }
 
 // OtA[r][p][a][l] = -ovoo[p][a][l][r]: one warp per ((r,p,a), K chunk)
+template <int MODE>
 __global__ void __launch_bounds__(256)
 pack_ota_kernel(const double* __restrict__ ovoo, int v, int o, int ok, uint32_t* __restrict__ OtA,
-                const float* __restrict__ scale_ptr) {
-    const double scale = (double)*scale_ptr;
-    const int lane = threadIdx.x & 31, nch = ok / 32;
+                const float* __restrict__ sc) {
+    constexpr int CW = MODE ? 64 : 32;
+    const double scale = pack_scale<MODE>(sc, 0);
+    const int lane = threadIdx.x & 31, nch = ok / CW;
     const size_t nw = (size_t)o * o * v * nch;
     for (size_t w = blockIdx.x * (size_t)8 + (threadIdx.x >> 5); w < nw; w += (size_t)gridDim.x * 8) {
         const size_t row = w / nch;                        // (r, p, a)
-        const int l = (int)(w % nch) * 32 + lane;
+        const int ch = (int)(w % nch), l = ch * 32 + lane;
         const int a = (int)(row % v), p = (int)((row / v) % o), r = (int)(row / ((size_t)v * o));
-        const float xs = l < o ? (float)(-ovoo[(((size_t)p * v + a) * o + l) * o + r] * scale) : 0.0f;
-        pack_split_store(OtA + row * ok + (l - lane), xs, lane);
+        const double x = l < o ? -ovoo[(((size_t)p * v + a) * o + l) * o + r] : 0.0;
+        pack_store<MODE>(OtA + row * ok + (size_t)ch * CW, x, scale, lane);
     }
 }
 

@@ -160,6 +160,21 @@ __device__ __forceinline__ void umma_f16_pair(uint32_t tmem_d, uint32_t adesc_lo
         ::"r"(tmem_d), "r"(adesc_lo), "r"(bdesc_lo), "r"(idesc), "r"(accumulate), "r"(UMMA_DESC_HI_SW128)
         : "memory");
 }
+// kind::i8 (K = 32 per instruction), signed 8-bit operands, S32 accumulate, M = 256 over the pair
+__device__ __forceinline__ uint32_t umma_idesc_s8_m256(uint32_t n) {
+    return (2u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((256u >> 4) << 24);
+}
+__device__ __forceinline__ void umma_i8_pair(uint32_t tmem_d, uint32_t adesc_lo, uint32_t bdesc_lo, uint32_t idesc,
+                                             uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "mov.b64 da, {%1, %5};\n\t"
+        "mov.b64 db, {%2, %5};\n\t"
+        "tcgen05.mma.cta_group::2.kind::i8 [%0], da, db, %3, p;\n\t}"
+        ::"r"(tmem_d), "r"(adesc_lo), "r"(bdesc_lo), "r"(idesc), "r"(accumulate), "r"(UMMA_DESC_HI_SW128)
+        : "memory");
+}
 // arrive on the barrier at this offset in both CTAs of the pair once every MMA issued so far has completed
 __device__ __forceinline__ void umma_commit_pair(uint64_t* bar) {
     asm volatile(

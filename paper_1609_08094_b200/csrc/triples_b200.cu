@@ -15,6 +15,7 @@
 #include <string>
 #include <vector>
 
+#include "gemm_emu64.cuh"
 #include "gemm_f16split.cuh"
 #include "gemm_f64.cuh"
 #include "plan.h"
@@ -177,6 +178,7 @@ struct Operands {   // device pointers of the repacked operands (workspace) for 
 struct Maps {   // tensor maps of the contraction kernel of the plan's precision
     GemmMaps f64;
     SplitMaps split;
+    EmuMaps emu;
     RiMaps ri;
 };
 
@@ -207,6 +209,20 @@ int build_maps_split(const Plan& P, const Operands& op, SplitMaps* maps) {
     return TRIPLES_OK;
 }
 
+// emulated-FP64 operands: 64 words (two 128-byte rows of digits) per K chunk; a box is one of the two rows
+int build_maps_emu(const Plan& P, const Operands& op, EmuMaps* maps) {
+    const uint64_t o = P.o, v = P.v, vk = P.vk, ok = P.ok, NR = (uint64_t)P.v * P.vp, ns = P.nslots;
+    const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_UINT32;
+    int rc;
+    if ((rc = make_map3(&maps->xk, dt, 4, op.x, vk, NR, ns, vk, NR * vk, 32, EM_BM, 1))) return rc;
+    if ((rc = make_map3(&maps->xkt, dt, 4, op.xt, vk, NR, ns, vk, NR * vk, 32, EM_BM, 1))) return rc;
+    if ((rc = make_map3(&maps->t2k, dt, 4, op.t2k, ok, NR, o, ok, NR * ok, 32, EM_BM, 1))) return rc;
+    if ((rc = make_map3(&maps->t2kt, dt, 4, op.t2kt, ok, NR, o, ok, NR * ok, 32, EM_BM, 1))) return rc;
+    if ((rc = make_map3(&maps->t2a, dt, 4, op.t2, vk, v, o * o, vk, v * vk, 32, EM_NPAD, 1))) return rc;
+    if ((rc = make_map3(&maps->ota, dt, 4, op.ot, ok, v, o * o, ok, v * ok, 32, EM_NPAD, 1))) return rc;
+    return TRIPLES_OK;
+}
+
 int build_maps_ri(const Plan& P, const Operands& op, RiMaps* maps) {
     const uint64_t v = P.v, vp = P.vp, o = P.o, na = P.naux, nap = P.nauxp;
     const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
@@ -219,23 +235,25 @@ int build_maps_ri(const Plan& P, const Operands& op, RiMaps* maps) {
 int build_maps(const Plan& P, const Operands& op, Maps* maps) {
     if (P.mode == SLICES_RI)
         if (int rc = build_maps_ri(P, op, &maps->ri)) return rc;
+    if (P.prec == TRIPLES_EMU64) return build_maps_emu(P, op, &maps->emu);
     return P.prec == TRIPLES_FP64 ? build_maps_f64(P, op, &maps->f64) : build_maps_split(P, op, &maps->split);
 }
 
-// co-resident CTA pairs of the mixed contraction, per (device, shared-memory request)
-int max_split_clusters(cudaLaunchConfig_t cfg, int cs, int* out) {
+// co-resident CTA pairs of a tcgen05 contraction kernel, per (kernel, device, shared-memory request)
+template <typename K>
+int max_pair_clusters(K kern, int which, cudaLaunchConfig_t cfg, int cs, int* out) {
     static std::mutex mu;
     static std::map<std::pair<int, size_t>, int> cache;
     int dev = 0;
     CU_TRY(cudaGetDevice(&dev));
     std::lock_guard<std::mutex> lk(mu);
-    const auto key = std::make_pair(dev, cfg.dynamicSmemBytes);
+    const auto key = std::make_pair(dev * 2 + which, cfg.dynamicSmemBytes);
     auto it = cache.find(key);
     if (it == cache.end()) {
         cfg.gridDim = dim3(kNumSM / cs * cs);
         int n = 0;
-        CU_TRY(cudaOccupancyMaxActiveClusters(&n, gemm_f16split_kernel, &cfg));
-        if (n < 1) return fail(TRIPLES_ECUDA, "no CTA pair of the mixed contraction fits the device");
+        CU_TRY(cudaOccupancyMaxActiveClusters(&n, kern, &cfg));
+        if (n < 1) return fail(TRIPLES_ECUDA, "no CTA pair of the tcgen05 contraction fits the device");
         it = cache.emplace(key, std::min(n, kNumSM / cs)).first;
     }
     *out = it->second;
@@ -259,7 +277,7 @@ int launch_gemm_split(const SplitMaps& maps, const GemmJob* jobs, int njobs, con
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     int max_clusters = 0;
-    if (int rc = max_split_clusters(cfg, cs, &max_clusters)) return rc;
+    if (int rc = max_pair_clusters(gemm_f16split_kernel, 0, cfg, cs, &max_clusters)) return rc;
     cfg.gridDim = dim3((unsigned)(std::min<long long>(items, max_clusters) * cs));
     CU_TRY(cudaLaunchKernelEx(&cfg, gemm_f16split_kernel, maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles, P.tf_ntiles,
                               P.tf_bn, P.tf_npad, scales));
@@ -267,8 +285,33 @@ int launch_gemm_split(const SplitMaps& maps, const GemmJob* jobs, int njobs, con
     return TRIPLES_OK;
 }
 
+int launch_gemm_emu(const EmuMaps& maps, const GemmJob* jobs, int njobs, const Plan& P, const float* scales,
+                    cudaStream_t st) {
+    CU_TRY(cudaFuncSetAttribute(gemm_emu64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, EM_SMEM_BYTES));
+    const int cs = P.tf_cs;
+    if (njobs > EM_MAX_JOBS) return fail(TRIPLES_EINVAL, "internal: %d contraction jobs in one launch (max %d)", njobs, EM_MAX_JOBS);
+    const long long items = (long long)njobs * ((P.tf_mtiles + cs - 1) / cs) * P.tf_ntiles;
+    if (items == 0) return TRIPLES_OK;
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cs; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.blockDim = dim3(EM_THREADS);
+    cfg.dynamicSmemBytes = EM_SMEM_BYTES;
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int max_clusters = 0;
+    if (int rc = max_pair_clusters(gemm_emu64_kernel, 1, cfg, cs, &max_clusters)) return rc;
+    cfg.gridDim = dim3((unsigned)(std::min<long long>(items, max_clusters) * cs));
+    CU_TRY(cudaLaunchKernelEx(&cfg, gemm_emu64_kernel, maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles, P.tf_ntiles, scales));
+    ++g_launches;
+    return TRIPLES_OK;
+}
+
 int launch_gemm(const Plan& P, const Maps& maps, const Operands& op, const GemmJob* jobs, int njobs, cudaStream_t st) {
     if (P.prec == TRIPLES_MIXED) return launch_gemm_split(maps.split, jobs, njobs, P, op.scales, st);
+    if (P.prec == TRIPLES_EMU64) return launch_gemm_emu(maps.emu, jobs, njobs, P, op.scales, st);
     switch (P.cfg) {
         case CFG_M120_N128: return launch_gemm_f64<3, 4, 4, 4>(maps.f64, jobs, njobs, P, st);
         case CFG_M80_N192: return launch_gemm_f64<2, 6, 4, 4>(maps.f64, jobs, njobs, P, st);
@@ -326,11 +369,11 @@ int transpose_slice(const Plan& P, const double* X, double* XT, cudaStream_t st)
 
 // src viewed as [d][s]: the resident vvvo (ro = o, slot = r) or one FP64 slice (ro = 1) -> packed XK / XKT slots
 int pack_xk(const Plan& P, const double* src, int ro, int sp, int slot0, const Operands& op, cudaStream_t st) {
-    CU_TRY(cudaFuncSetAttribute(pack_xk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PKX_SMEM));
+    auto kern = P.prec == TRIPLES_EMU64 ? pack_xk_kernel<1> : pack_xk_kernel<0>;
+    CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, PKX_SMEM));
     const size_t S = (size_t)P.v * P.v * ro;
-    dim3 grid((unsigned)((S + PKX_SPAN - 1) / PKX_SPAN), P.vk / 32);
-    pack_xk_kernel<<<grid, 256, PKX_SMEM, st>>>(src, P.v, P.vp, P.vk, ro, sp, slot0, (uint32_t*)op.x, (uint32_t*)op.xt,
-                                                op.scales);
+    dim3 grid((unsigned)((S + PKX_SPAN - 1) / PKX_SPAN), P.vk / P.kwords);
+    kern<<<grid, 256, PKX_SMEM, st>>>(src, P.v, P.vp, P.vk, ro, sp, slot0, (uint32_t*)op.x, (uint32_t*)op.xt, op.scales);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     return TRIPLES_OK;
@@ -341,8 +384,8 @@ int run_prepare(const Plan& P, const Inputs& in, const Source& src, const Operan
                 cudaStream_t copy_st) {
     const int o = P.o, v = P.v;
     if (P.vp != v) {   // pad rows / columns c = v stay zero (never written by the repack kernels)
-        CU_TRY(cudaMemsetAsync(op.x, 0, P.n_x * P.esz, st));
-        CU_TRY(cudaMemsetAsync(op.xt, 0, P.n_x * P.esz, st));
+        CU_TRY(cudaMemsetAsync(op.x, 0, P.n_x * P.osz, st));
+        CU_TRY(cudaMemsetAsync(op.xt, 0, P.n_x * P.osz, st));
         if (P.prec == TRIPLES_FP64) CU_TRY(cudaMemsetAsync(op.t2, 0, P.n_t2 * 8, st));
     }
     if (P.prec == TRIPLES_FP64) {
@@ -369,7 +412,8 @@ int run_prepare(const Plan& P, const Inputs& in, const Source& src, const Operan
         ++g_launches;
         return TRIPLES_OK;
     }
-    // ---- mixed path
+    // ---- packed paths (mixed: FP16 split; emulated FP64: base-128 digits)
+    const bool emu = P.prec == TRIPLES_EMU64;
     if (P.vp != v) {
         CU_TRY(cudaMemsetAsync(op.t2k, 0, P.n_t2k * 4, st));
         CU_TRY(cudaMemsetAsync(op.t2kt, 0, P.n_t2k * 4, st));
@@ -415,14 +459,16 @@ int run_prepare(const Plan& P, const Inputs& in, const Source& src, const Operan
         if (int rc = pack_xk(P, src.vvvo, o, v, 0, op, st)) return rc;
     {
         dim3 grid(o * v, (v + 63) / 64, (o + 63) / 64);
-        pack_t2k_kernel<<<grid, 256, 0, st>>>(in.t2, v, P.vp, o, P.ok, (uint32_t*)op.t2k, (uint32_t*)op.t2kt, op.scales + 1);
+        (emu ? pack_t2k_kernel<1> : pack_t2k_kernel<0>)<<<grid, 256, 0, st>>>(in.t2, v, P.vp, o, P.ok, (uint32_t*)op.t2k,
+                                                                               (uint32_t*)op.t2kt, op.scales);
         CU_TRY(cudaGetLastError());
         ++g_launches;
     }
-    pack_ota_kernel<<<kNumSM * 4, 256, 0, st>>>(in.ovoo, v, o, P.ok, (uint32_t*)op.ot, op.scales);
+    (emu ? pack_ota_kernel<1> : pack_ota_kernel<0>)<<<kNumSM * 4, 256, 0, st>>>(in.ovoo, v, o, P.ok, (uint32_t*)op.ot, op.scales);
     CU_TRY(cudaGetLastError());
     ++g_launches;
-    pack_t2a_kernel<<<kNumSM * 8, 256, 0, st>>>(in.t2, (size_t)o * o * v, v, P.vk, (uint32_t*)op.t2, op.scales + 1);
+    (emu ? pack_t2a_kernel<1> : pack_t2a_kernel<0>)<<<kNumSM * 8, 256, 0, st>>>(in.t2, (size_t)o * o * v, v, P.vk,
+                                                                                 (uint32_t*)op.t2, op.scales);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     return TRIPLES_OK;
@@ -431,7 +477,7 @@ int run_prepare(const Plan& P, const Inputs& in, const Source& src, const Operan
 Operands carve_operands(const Plan& P, uint8_t* ws) {
     Operands op{};
     op.x = ws + P.off_x; op.xt = ws + P.off_xt; op.ot = ws + P.off_ot; op.t2 = ws + P.off_t2;
-    if (P.prec == TRIPLES_MIXED) {
+    if (P.prec != TRIPLES_FP64) {
         op.t2k = ws + P.off_t2k; op.t2kt = ws + P.off_t2kt;
         op.scales = reinterpret_cast<float*>(ws + P.off_result + 64);   // the result block has 256 bytes, 24 used
     }
@@ -693,7 +739,7 @@ int check_device_inputs(const void* const* ptrs, int nptr, const void* ws) {
 
 int dispatch_batches(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws, cudaStream_t st,
                      const std::vector<Triplet>& trip, double* e_trip, size_t rows, const RunOpts& opt = RunOpts()) {
-    if (P.prec == TRIPLES_FP64) return run_batches<double>(P, in, src, ws, st, trip, e_trip, rows, opt);
+    if (P.prec != TRIPLES_MIXED) return run_batches<double>(P, in, src, ws, st, trip, e_trip, rows, opt);
     return run_batches<float>(P, in, src, ws, st, trip, e_trip, rows, opt);
 }
 
@@ -1039,7 +1085,7 @@ int triples_w_block(int nocc, int nvirt, const double* t2, const double* vvvo, c
     GemmJob* d_gj = reinterpret_cast<GemmJob*>(ws + P.off_gjobs);
     CU_TRY(cudaMemcpyAsync(d_gj, gj, sizeof gj, cudaMemcpyHostToDevice, st));
     if (int rc = launch_gemm(P, maps, op, d_gj, 3, st)) return rc;
-    if (precision == TRIPLES_FP64)
+    if (P.esz == 8)
         assemble_w_kernel<double><<<kNumSM * 4, 256, 0, st>>>((const double*)ubase, nvirt, P.nt, W_out);
     else
         assemble_w_kernel<float><<<kNumSM * 4, 256, 0, st>>>((const float*)ubase, nvirt, P.nt, W_out);

@@ -12,7 +12,7 @@ from paper_1609_08094_b200 import synth
 
 pytestmark = pytest.mark.gpu
 
-TOL = {tb.FP64: 1e-10, tb.MIXED: 1e-5}
+TOL = {tb.FP64: 1e-10, tb.MIXED: 1e-5, tb.EMU64: 1e-10}
 NAMES = ("eps_o", "eps_v", "t1", "t2", "vvvo", "ovoo", "ovov")
 
 
@@ -156,6 +156,45 @@ def test_tiny_config_full_parity_mixed(seed, t1_sigma):
         assert rel(E[n], Eo[n]) <= TOL[tb.MIXED], (n, E, Eo)
     assert np.abs(et - et_o).max() <= TOL[tb.MIXED] * np.abs(et_o).max()
     assert rel(et[:, 0].sum(), E[0]) <= 1e-13
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# emulated-FP64 path (INT8 tensor cores, seven base-128 digits per operand) against the FP64 oracle
+# at the FP64 tolerance
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("o,v,naux,ijk", [
+    (3, 5, 9, (0, 1, 2)), (3, 5, 9, (1, 1, 0)), (4, 17, 20, (3, 0, 2)), (5, 41, 50, (4, 2, 0)),
+    (3, 50, 40, (0, 1, 2)), (6, 96, 60, (5, 1, 3)), (4, 130, 50, (1, 3, 2)), (8, 40, 120, (7, 3, 5)),
+    (17, 24, 30, (16, 0, 9)), (35, 20, 40, (33, 0, 34)), (16, 160, 30, (5, 2, 11)),
+])
+def test_w_block_elementwise_emu64(o, v, naux, ijk):
+    """Exact integer digit products, levels <= 6 kept: W within 1e-11 of the oracle on the scale of W (the dropped
+    levels are < 2^-44 of (class maximum)^2 per term; K = 2v + 2o terms)."""
+    inp = synth.make_inputs(o, v, naux, seed=3)
+    d = to_dev(inp)
+    ws = workspace(o, v, tb.EMU64)
+    W = torch.full((v, v, v), float("nan"), dtype=torch.float64, device="cuda")
+    tb.triples_w_block(o, v, d[3], d[4], d[5], tb.EMU64, *ijk, ws, W)
+    Wo = oracle.w_block(o, v, inp.t2, inp.vvvo, inp.ovoo, *ijk)
+    err = np.abs(W.cpu().numpy() - Wo).max()
+    assert err <= 1e-11 * np.abs(Wo).max(), f"max abs err {err:.3e} vs scale {np.abs(Wo).max():.3e}"
+
+
+@pytest.mark.parametrize("o,v,naux,t1_sigma", [
+    (2, 3, 5, 0.3), (3, 5, 9, 0.3), (4, 16, 30, 0.3), (3, 17, 30, 0.3), (5, 41, 60, 0.3), (6, 24, 40, 1.0),
+    (7, 33, 40, 1e-3), (1, 6, 8, 0.3), (8, 40, 120, 1e-3),
+])
+def test_energy_small_cases_emu64(o, v, naux, t1_sigma):
+    inp = synth.make_inputs(o, v, naux, seed=1, t1_sigma=t1_sigma)
+    (E, et) = gpu_energy(inp, prec=tb.EMU64, with_triplets=True)
+    (Eo, et_o) = oracle.energy_restricted(o, v, *inp.arrays(), with_triplets=True)
+    if o == 1:
+        assert E == (0.0, 0.0, 0.0)
+        return
+    scale = abs(Eo[1])
+    for n in range(3):
+        assert abs(E[n] - Eo[n]) <= TOL[tb.EMU64] * max(abs(Eo[n]), 1e-3 * scale), (n, E, Eo)
+    assert np.abs(et - et_o).max() <= TOL[tb.EMU64] * np.abs(et_o).max()
 
 
 # ------------------------------------------------------------------------------------------------------------------
