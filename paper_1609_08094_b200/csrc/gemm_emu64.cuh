@@ -4,20 +4,23 @@
 // the 37 TFLOP/s FP64 tensor peak) and the FP16-split path (gemm_f16split.cuh).
 //
 // Ozaki-style error-free slicing with ONE power-of-two scale per tensor class (as on the mixed path): every operand
-// is the 49-bit fixed-point integer xi = rint(x 2^(s+33)) = sum_i d_i 128^(6-i), seven balanced base-128 digits
+// is the 42-bit fixed-point integer xi = rint(x 2^(s+26)) = sum_i d_i 128^(5-i), six balanced base-128 digits
 // d_i in [-64, 63] (prepare.cuh pack_emu_store).  Then
-//     sum_k xi_k yi_k = sum_{i,j} 128^(12-i-j) S_ij,   S_ij = sum_k d_i(x_k) d_j(y_k)   (an exact int8 x int8 -> int32 GEMM)
+//     sum_k xi_k yi_k = sum_{i,j} 128^(10-i-j) S_ij,   S_ij = sum_k d_i(x_k) d_j(y_k)   (an exact int8 x int8 -> int32 GEMM)
 // and the pairs of one LEVEL L = i + j share a weight, so they accumulate in ONE int32 TMEM accumulator: (L+1) K 64^2
-// < 2^31 for K <= 74000.  Levels L <= 6 are kept (28 digit products per K chunk); the dropped levels are below
-// 2^-44 of (class maximum)^2 per term.  Integer accumulation is exact, so -- unlike the FP16-split kernel -- a whole
-// work item (all four K segments) accumulates in TMEM and is read out once: S_L -> double, W = sum_L S_L c_L with the
-// exact powers of two c_L = 2^(7(12-L) - (sg+st) - 66); seven FMAs per element, rounding ~1e-16.
+// < 2^31 for K <= 87000.  Levels L <= 5 are kept (21 digit products per 32 K elements); the dropped levels are below
+// 2^-38 of (class maximum)^2 per term, of the order of the 2^-40 quantisation of the operands themselves.  Integer
+// accumulation is exact, so -- unlike the FP16-split kernel -- a whole work item (all four K segments) accumulates in
+// TMEM and is read out once: S_L -> double, W = sum_L S_L c_L with the exact powers of two
+// c_L = 2^(7(10-L) - (sg+st) - 52); six FMAs per element, rounding ~1e-16.  (A first version with seven digits and
+// levels <= 6 -- 28 products, BN = 64 -- measured 2e-14 per-triplet parity and 73 TFLOP/s at medium.)
 //
 // Same G job, tiling and roles as gemm_f16split.cuh (transposed: the (b,c) index is the MMA's M dimension, CTA pairs,
-// 128 TMEM lanes per CTA), with BN = 64 a-columns per tile: seven level accumulators of 64 columns = 448 of the 512
-// TMEM columns.  Operands: per row and 32-wide K chunk two 128-byte rows (digits 0..3 | digits 4..6, 32 bytes each),
-// staged by TMA with SWIZZLE_128B; an MMA reads digit i of the M side and digit j of the N side through descriptors
-// advanced by 32 bytes per digit.  Output: the FP64 U buffers of ulayout.cuh, reduced by reduce_kernel<double>.
+// 128 TMEM lanes per CTA), with BN = 80 a-columns per tile: six level accumulators of 80 columns = 480 of the 512
+// TMEM columns.  K is walked in chunks of 64: per operand row three 128-byte rows of digit pairs (prepare.cuh), staged
+// by TMA with SWIZZLE_128B; an MMA (K = 32) reads digit i of the M side and digit j of the N side for one half of the
+// chunk through descriptors advanced by 64 bytes per digit and 32 bytes per half.  Output: the FP64 U buffers of
+// ulayout.cuh, reduced by reduce_kernel<double>.
 #pragma once
 #include "gemm_f64.cuh"   // GemmJob, grouped_item
 #include "ptx.cuh"
@@ -27,20 +30,22 @@ namespace tb {
 
 struct alignas(64) EmuMaps {
     CUtensorMap xk, xkt, t2k, t2kt;   // M side: (word, n = (b,c'), slot | q | r)      box (32, 128, 1)
-    CUtensorMap t2a, ota;             // N side: (word, a, p*o+q | r*o+p)              box (32, 32, 1)
+    CUtensorMap t2a, ota;             // N side: (word, a, p*o+q | r*o+p)              box (32, 40, 1)
 };
 
 constexpr int EM_BM = 128;            // (b,c) rows per CTA tile = TMEM lanes
-constexpr int EM_BN = 64;             // a-columns per tile
+constexpr int EM_BN = 80;             // a-columns per tile
 constexpr int EM_NPAD = EM_BN / 2;    // N-side rows a CTA stages
-constexpr int EM_DIGITS = 7;
-constexpr int EM_LEVELS = 7;          // levels 0..6 kept
-constexpr int EM_CW = 64;             // 4-byte words per operand row and K chunk (two 128-byte rows)
+constexpr int EM_DIGITS = 6;
+constexpr int EM_LEVELS = 6;          // levels 0..5 kept
+constexpr int EM_BK = 64;             // K elements per chunk
+constexpr int EM_CW = 96;             // 4-byte words per operand row and K chunk (three 128-byte rows of digit pairs)
+constexpr int EM_ROWS = 3;
 constexpr int EM_THREADS = 384;
 constexpr int EM_ACC_WARP0 = 4;
 constexpr int EM_TMEM_COLS = 512;
-constexpr int EM_STAGES = 5;
-constexpr int EM_TILE_BYTES = 2 * (EM_BM + EM_NPAD) * 128;      // 40 KB: [M lo][M hi][N lo][N hi]
+constexpr int EM_STAGES = 3;
+constexpr int EM_TILE_BYTES = EM_ROWS * (EM_BM + EM_NPAD) * 128;      // 63 KB: [M row 0..2][N row 0..2]
 constexpr int EM_MAX_JOBS = 192;
 constexpr int EM_TAIL_BYTES = 2048 + EM_MAX_JOBS * 48;
 constexpr int EM_SMEM_BYTES = EM_STAGES * EM_TILE_BYTES + EM_TAIL_BYTES;
@@ -67,7 +72,7 @@ gemm_emu64_kernel(const __grid_constant__ EmuMaps maps, const GemmJob* __restric
     const int cid = blockIdx.x / cs, ncl = gridDim.x / cs;
     const int per_job = ((mtiles + cs - 1) / cs) * ntiles;
     const long long nitems = (long long)njobs * per_job;
-    const int nch_v = (v + 31) / 32, nch_o = (o + 31) / 32;
+    const int nch_v = (v + EM_BK - 1) / EM_BK, nch_o = (o + EM_BK - 1) / EM_BK;
     const int nch = 2 * (nch_v + nch_o);
 
     if (threadIdx.x == 0) {
@@ -101,7 +106,7 @@ gemm_emu64_kernel(const __grid_constant__ EmuMaps maps, const GemmJob* __restric
                     const int s = it % EM_STAGES;
                     mbar_wait(&empty[s], ((it / EM_STAGES) & 1) ^ 1);
                     uint8_t* sM = smem + s * EM_TILE_BYTES;
-                    uint8_t* sN = sM + 2 * EM_BM * 128;
+                    uint8_t* sN = sM + EM_ROWS * EM_BM * 128;
                     if (rank == 0) mbar_arrive_expect_tx(&full[s], 2 * EM_TILE_BYTES);
                     const CUtensorMap *mm, *nm;
                     int kk, mz, nz;
@@ -110,10 +115,11 @@ gemm_emu64_kernel(const __grid_constant__ EmuMaps maps, const GemmJob* __restric
                     else if (c < 2 * nch_v + nch_o)    { kk = (c - 2 * nch_v) * EM_CW;         mm = &maps.t2k;  mz = q;      nm = &maps.ota; nz = r * o + p; }
                     else                               { kk = (c - 2 * nch_v - nch_o) * EM_CW; mm = &maps.t2kt; mz = r;      nm = &maps.ota; nz = q * o + p; }
                     const uint32_t bar = lfull0 + 8u * s;
-                    tma_load_3d_pair(sM, mm, bar, kk, m0, mz);
-                    tma_load_3d_pair(sM + EM_BM * 128, mm, bar, kk + 32, m0, mz);
-                    tma_load_3d_pair(sN, nm, bar, kk, an, nz);
-                    tma_load_3d_pair(sN + EM_NPAD * 128, nm, bar, kk + 32, an, nz);
+#pragma unroll
+                    for (int pr = 0; pr < EM_ROWS; ++pr) {
+                        tma_load_3d_pair(sM + pr * EM_BM * 128, mm, bar, kk + 32 * pr, m0, mz);
+                        tma_load_3d_pair(sN + pr * EM_NPAD * 128, nm, bar, kk + 32 * pr, an, nz);
+                    }
                 }
             }
         }
@@ -131,20 +137,36 @@ gemm_emu64_kernel(const __grid_constant__ EmuMaps maps, const GemmJob* __restric
                     const int s = it % EM_STAGES;
                     mbar_wait(&full[s], (it / EM_STAGES) & 1);
                     tc_fence_after_sync();
+                    int left;   // K elements of this chunk's segment from the chunk start
+                    if (c < nch_v) left = v - c * EM_BK;
+                    else if (c < 2 * nch_v) left = v - (c - nch_v) * EM_BK;
+                    else if (c < 2 * nch_v + nch_o) left = o - (c - 2 * nch_v) * EM_BK;
+                    else left = o - (c - 2 * nch_v - nch_o) * EM_BK;
+                    const bool two = left > 32;                    // the second half of the chunk carries data
                     if (issuer) {
                         const uint32_t t0 = smem_base + s * EM_TILE_BYTES;
-                        const uint32_t mlo = umma_desc_lo(t0), mhi = umma_desc_lo(t0 + EM_BM * 128);
-                        const uint32_t nlo = umma_desc_lo(t0 + 2 * EM_BM * 128);
-                        const uint32_t nhi = umma_desc_lo(t0 + 2 * EM_BM * 128 + EM_NPAD * 128);
+                        uint32_t md[EM_ROWS], nd[EM_ROWS];
+#pragma unroll
+                        for (int pr = 0; pr < EM_ROWS; ++pr) {
+                            md[pr] = umma_desc_lo(t0 + pr * EM_BM * 128);
+                            nd[pr] = umma_desc_lo(t0 + EM_ROWS * EM_BM * 128 + pr * EM_NPAD * 128);
+                        }
                         const uint32_t fresh = c == 0 ? 0u : 1u;
 #pragma unroll
-                        for (int i = 0; i < EM_DIGITS; ++i) {
-                            const uint32_t ad = (i < 4 ? mlo + 2 * i : mhi + 2 * (i - 4));     // 32 bytes per digit
+                        for (int h = 0; h < 2; ++h) {
+                            if (h == 0 || two) {
 #pragma unroll
-                            for (int j = 0; i + j < EM_LEVELS; ++j) {
-                                const uint32_t bd = (j < 4 ? nlo + 2 * j : nhi + 2 * (j - 4));
-                                // level L = i + j; its first product of the item (i = 0, chunk 0) overwrites
-                                umma_i8_pair(tmem_base + (uint32_t)(i + j) * EM_BN, ad, bd, idesc, i == 0 ? fresh : 1u);
+                                for (int i = 0; i < EM_DIGITS; ++i) {
+                                    const uint32_t ad = md[i >> 1] + 4 * (i & 1) + 2 * h;   // 64 B per digit, 32 B per half
+#pragma unroll
+                                    for (int j = 0; i + j < EM_LEVELS; ++j) {
+                                        const uint32_t bd = nd[j >> 1] + 4 * (j & 1) + 2 * h;
+                                        // level L = i + j; its first product of the item (i = 0, first half of chunk 0)
+                                        // overwrites the accumulator
+                                        umma_i8_pair(tmem_base + (uint32_t)(i + j) * EM_BN, ad, bd, idesc,
+                                                     (i == 0 && h == 0) ? fresh : 1u);
+                                    }
+                                }
                             }
                         }
                         umma_commit_pair(&empty[s]);
@@ -157,23 +179,24 @@ gemm_emu64_kernel(const __grid_constant__ EmuMaps maps, const GemmJob* __restric
     } else if (warp >= EM_ACC_WARP0) {
         // ------------------------------------------------------------------------------------ accumulator warps
         const int wq = warp & 3;                            // TMEM lane quarter this warp may read
-        const int half = (warp - EM_ACC_WARP0) >> 2;        // columns [32*half, 32*half + 32) of every level
+        constexpr int HC = EM_BN / 2;                       // columns per warp
+        const int half = (warp - EM_ACC_WARP0) >> 2;        // columns [40*half, 40*half + 40) of every level
         const uint32_t ltempty = mapa_u32(smem_u32(&tempty[0]), 0);
-        const int sexp = reinterpret_cast<const int*>(scales)[12] + reinterpret_cast<const int*>(scales)[13] + 66;
+        const int sexp = reinterpret_cast<const int*>(scales)[12] + reinterpret_cast<const int*>(scales)[13] + 52;
         uint32_t item = 0;
         for (long long w = cid; w < nitems; w += ncl, ++item) {
             int jb, rem;
             grouped_item(jobs, w, per_job, jb, rem);
-            const int m0 = ((rem / ntiles) * cs + rank) * EM_BM, a0 = (rem % ntiles) * EM_BN + half * 32;
-            double acc[32];
+            const int m0 = ((rem / ntiles) * cs + rank) * EM_BM, a0 = (rem % ntiles) * EM_BN + half * HC;
+            double acc[HC];
 #pragma unroll
-            for (int j = 0; j < 32; ++j) acc[j] = 0.0;
+            for (int j = 0; j < HC; ++j) acc[j] = 0.0;
             mbar_wait(&tfull[0], item & 1);
             tc_fence_after_sync();
 #pragma unroll
             for (int L = 0; L < EM_LEVELS; ++L) {
-                const double cL = ldexp(1.0, 7 * (12 - L) - sexp);       // exact power of two
-                const uint32_t taddr = tmem_base + (uint32_t)L * EM_BN + half * 32 + ((uint32_t)(wq * 32) << 16);
+                const double cL = ldexp(1.0, 7 * (10 - L) - sexp);       // exact power of two
+                const uint32_t taddr = tmem_base + (uint32_t)L * EM_BN + half * HC + ((uint32_t)(wq * 32) << 16);
 #pragma unroll
                 for (int c0 = 0; c0 < 32; c0 += 16) {
                     uint32_t rg[16];
@@ -181,6 +204,13 @@ gemm_emu64_kernel(const __grid_constant__ EmuMaps maps, const GemmJob* __restric
                     tmem_ld_wait();
 #pragma unroll
                     for (int j = 0; j < 16; ++j) acc[c0 + j] = fma((double)(int)rg[j], cL, acc[c0 + j]);
+                }
+                {
+                    uint32_t rg[8];
+                    tmem_ld_32x32b_x8(taddr + 32, rg);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) acc[32 + j] = fma((double)(int)rg[j], cL, acc[32 + j]);
                 }
             }
             tc_fence_before_sync();
@@ -196,7 +226,7 @@ gemm_emu64_kernel(const __grid_constant__ EmuMaps maps, const GemmJob* __restric
                 const size_t astride = (size_t)nt * nt * UCHUNK;   // one a-tile
                 const size_t cb = ((size_t)(bb >> 3) * nt + (cc >> 3)) * UCHUNK + u_swz<8>(0, bb & 7, cc & 7);
 #pragma unroll
-                for (int j = 0; j < 32; ++j) {
+                for (int j = 0; j < HC; ++j) {
                     if (a0 + j < v) {
                         const size_t off = (size_t)((a0 + j) >> 3) * astride + (cb ^ (size_t)u_swz<8>(j & 7, 0, 0));
                         out[off] = acc[j];

@@ -88,7 +88,7 @@ struct Plan {
     size_t off_side = 0;
     size_t esz = 8;             // bytes per stored U element (FP64 / emulated FP64: 8, mixed: 4)
     size_t osz = 8;             // bytes per stored operand word (FP64: 8; mixed and emulated FP64: 4-byte packed words)
-    int kwords = 32;            // packed paths: 4-byte words per operand row and 32-wide K chunk (mixed 32, emulated 64)
+    int kchunks_v = 0, kchunks_o = 0;   // packed paths: 32-element K chunks a virtual / occupied operand row holds
     size_t n_x = 0, n_ot = 0, n_t2 = 0, n_u = 0;   // elements of one X (or XT), Ot, T2, one U buffer
     size_t n_t2k = 0;                              // mixed: elements of T2K (or T2KT)
     size_t off_t2k = 0, off_t2kt = 0;
@@ -126,7 +126,6 @@ inline bool make_plan(int o, int v, int prec, Plan& P, int mode = SLICES_RESIDEN
     P.op = (o + 1) & ~1;
     P.esz = prec == 1 ? 4 : 8;
     P.osz = prec == 0 ? 8 : 4;
-    P.kwords = prec == 2 ? 64 : 32;
     P.T = triplet_count(o);
     P.norb = (int)orbit_count(v);
     // CTA tile: the M tile (40, 80 or 120 rows) that wastes the fewest padded rows; ties -> larger tile
@@ -148,10 +147,17 @@ inline bool make_plan(int o, int v, int prec, Plan& P, int mode = SLICES_RESIDEN
     P.n_u = (size_t)P.nt * P.nt * P.nt * 512;          // blocked layout of ulayout.cuh
     P.n_side = (size_t)P.nt * P.nt * 448;             // tile-pair records of reduce.cuh
     if (prec != 0) {   // packed K-major operands, transposed tiles (gemm_f16split.cuh / gemm_emu64.cuh)
-        P.vk = ((v + 31) / 32) * P.kwords;     // whole 32-wide K chunks (one / two 128-byte packed rows each)
-        P.ok = ((o + 31) / 32) * P.kwords;
-        P.tf_ntiles = prec == 1 ? (v + 255) / 256 : (v + 63) / 64;
-        P.tf_bn = prec == 1 ? ((((v + P.tf_ntiles - 1) / P.tf_ntiles) + 15) & ~15) : 64;
+        if (prec == 1) {       // FP16 split: 32 words (one 128-byte row) per 32-wide K chunk
+            P.vk = (v + 31) / 32 * 32; P.ok = (o + 31) / 32 * 32;
+            P.kchunks_v = P.vk / 32; P.kchunks_o = P.ok / 32;
+            P.tf_ntiles = (v + 255) / 256;
+            P.tf_bn = (((v + P.tf_ntiles - 1) / P.tf_ntiles) + 15) & ~15;
+        } else {               // emulated FP64: 96 words (three 128-byte rows of digit pairs) per 64-wide K chunk
+            P.vk = (v + 63) / 64 * 96; P.ok = (o + 63) / 64 * 96;
+            P.kchunks_v = P.vk / 96 * 2; P.kchunks_o = P.ok / 96 * 2;
+            P.tf_bn = 80;
+            P.tf_ntiles = (v + 79) / 80;
+        }
         P.tf_mtiles = (int)((N + 127) / 128);
         // CTA pairs (cta_group::2): a pair owns two consecutive m-tiles, each CTA stages half of the N-side rows
         // (tf_bn is a multiple of 16, so a half is whole 8-row swizzle atoms)

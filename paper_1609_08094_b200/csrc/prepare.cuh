@@ -131,32 +131,39 @@ __device__ __forceinline__ void pack_split_store(uint32_t* __restrict__ row, flo
     row[(lane >> 1) + (odd ? 16 : 0)] = odd ? (got | (mine << 16)) : (mine | (got << 16));
 }
 
-// Emulated-FP64 path (gemm_emu64.cuh): the scaled value is rounded to a 49-bit fixed-point integer
-// xi = rint(x * 2^(s + 33)) (|xi| < 2^47: the class maximum sits in [2^46, 2^47)) and cut into seven balanced base-128
-// digits d_0 (most significant) .. d_6 in [-64, 63], xi = sum_i d_i 128^(6-i).  Per operand row and 32-wide K chunk TWO
-// 128-byte rows: bytes [32 i, 32 i + 32) of the first hold digit i = 0..3 of the 32 K elements, of the second digit
-// i = 4..6 (the last 32 bytes are zero).  The 32 lanes of a warp hold 32 consecutive K elements.
-constexpr int EMU_SHIFT = 33;
-__device__ __forceinline__ void pack_emu_store(uint32_t* __restrict__ row2, double x, int lane) {
+// Emulated-FP64 path (gemm_emu64.cuh): the scaled value is rounded to a 42-bit fixed-point integer
+// xi = rint(x * 2^(s + 26)) (|xi| < 2^40: the class maximum sits in [2^39, 2^40)) and cut into six balanced base-128
+// digits d_0 (most significant) .. d_5 in [-64, 63], xi = sum_i d_i 128^(5-i).  K is walked in chunks of 64; per
+// operand row and chunk THREE 128-byte rows (96 words): row p holds digit 2p of the 64 K elements in bytes 0..63 and
+// digit 2p+1 in bytes 64..127 -- 6 bytes per element, no padding.  The 32 lanes of a warp hold 32 consecutive K
+// elements = half h of a chunk.
+constexpr int EMU_SHIFT = 26;
+constexpr int EMU_DIGITS = 6;
+constexpr int EMU_CHUNK_WORDS = 96;
+__device__ __forceinline__ void pack_emu_store(uint32_t* __restrict__ chunk, int h, double x, int lane) {
     long long xi = __double2ll_rn(x);
-    int8_t d[8];
+    int8_t d[EMU_DIGITS];
 #pragma unroll
-    for (int i = 6; i >= 0; --i) {
+    for (int i = EMU_DIGITS - 1; i >= 0; --i) {
         int r = (int)(xi & 127);
         if (r >= 64) r -= 128;
         d[i] = (int8_t)r;
         xi = (xi - r) >> 7;
     }
-    d[7] = 0;
-    int8_t* b = reinterpret_cast<int8_t*>(row2);
+    int8_t* b = reinterpret_cast<int8_t*>(chunk);
 #pragma unroll
-    for (int i = 0; i < 8; ++i) b[(i >> 2) * 128 + (i & 3) * 32 + lane] = d[i];
+    for (int i = 0; i < EMU_DIGITS; ++i) b[(i >> 1) * 128 + (i & 1) * 64 + h * 32 + lane] = d[i];
 }
-// one packed K chunk of one operand row: MODE 0 = FP16 split (32 words), MODE 1 = emulated FP64 digits (64 words)
+// K chunk ch (32 elements) of the operand row starting at `row`: MODE 0 = FP16 split (32 words per chunk),
+// MODE 1 = emulated-FP64 digits (96 words per pair of chunks)
 template <int MODE>
-__device__ __forceinline__ void pack_store(uint32_t* __restrict__ row, double x, double scale, int lane) {
-    if constexpr (MODE == 0) pack_split_store(row, (float)(x * scale), lane);
-    else pack_emu_store(row, x * scale, lane);
+__device__ __forceinline__ void pack_store(uint32_t* __restrict__ row, int ch, double x, double scale, int lane) {
+    if constexpr (MODE == 0) pack_split_store(row + (size_t)ch * 32, (float)(x * scale), lane);
+    else pack_emu_store(row + (size_t)(ch >> 1) * EMU_CHUNK_WORDS, ch & 1, x * scale, lane);
+}
+// 32-element K chunks a row of pitch `words` holds
+template <int MODE> __device__ __forceinline__ int pack_chunks(int words) {
+    return MODE == 0 ? words / 32 : 2 * (words / EMU_CHUNK_WORDS);
 }
 // scale of a tensor class: sc = the scales block of prepare (floats 2^sg, 2^st, .. ; ints sg, st at [12], [13])
 template <int MODE>
@@ -176,7 +183,6 @@ template <int MODE>
 __global__ void __launch_bounds__(256)
 pack_xk_kernel(const double* __restrict__ src, int v, int vp, int vk, int ro, int sp, int slot0,
                uint32_t* __restrict__ XK, uint32_t* __restrict__ XKT, const float* __restrict__ sc) {
-    constexpr int CW = MODE ? 64 : 32;               // words per K chunk
     const double scale = pack_scale<MODE>(sc, 0);
     extern __shared__ double tile[];                 // [32][PKX_PITCH]
     const int d0 = blockIdx.y * 32;
@@ -200,9 +206,9 @@ pack_xk_kernel(const double* __restrict__ src, int v, int vp, int vk, int ro, in
         const size_t bc = sg / ro;
         const int b = (int)(bc / v), c = (int)(bc % v);
         const double x = tile[lane * PKX_PITCH + s];
-        const size_t base = (size_t)(slot0 + r) * plane + (size_t)blockIdx.y * CW;
-        pack_store<MODE>(XK + base + ((size_t)b * vp + c) * vk, x, scale, lane);
-        pack_store<MODE>(XKT + base + ((size_t)c * vp + b) * vk, x, scale, lane);
+        const size_t base = (size_t)(slot0 + r) * plane;
+        pack_store<MODE>(XK + base + ((size_t)b * vp + c) * vk, blockIdx.y, x, scale, lane);
+        pack_store<MODE>(XKT + base + ((size_t)c * vp + b) * vk, blockIdx.y, x, scale, lane);
     }
 }
 
@@ -212,7 +218,6 @@ template <int MODE>
 __global__ void __launch_bounds__(256)
 pack_t2k_kernel(const double* __restrict__ t2, int v, int vp, int o, int ok, uint32_t* __restrict__ T2K,
                 uint32_t* __restrict__ T2KT, const float* __restrict__ sc) {
-    constexpr int CW = MODE ? 64 : 32;
     const double scale = pack_scale<MODE>(sc, 1);
     __shared__ double tile[64][65];
     const int q = blockIdx.x / v, x = blockIdx.x % v;
@@ -226,11 +231,11 @@ pack_t2k_kernel(const double* __restrict__ t2, int v, int vp, int o, int ok, uin
     const int lane = threadIdx.x & 31;
     for (int e = threadIdx.x; e < 64 * ny; e += 256) {       // a warp = 32 consecutive l of one y
         const int lh = (e >> 5) & 1, yy = e >> 6;
-        const int l = (l0 / 32 + lh) * CW;                   // word offset of this K chunk in a row
-        if (l >= ok) continue;                               // warp-uniform
+        const int ch = l0 / 32 + lh;                         // 32-element K chunk of the row
+        if (ch >= pack_chunks<MODE>(ok)) continue;           // warp-uniform
         const double xv = tile[lh * 32 + lane][yy];
-        pack_store<MODE>(T2K + (((size_t)q * v + x) * vp + (y0 + yy)) * ok + l, xv, scale, lane);     // T2K [q][b=x][c=y][l]
-        pack_store<MODE>(T2KT + (((size_t)q * v + (y0 + yy)) * vp + x) * ok + l, xv, scale, lane);    // T2KT[q][b=y][c=x][l]
+        pack_store<MODE>(T2K + (((size_t)q * v + x) * vp + (y0 + yy)) * ok, ch, xv, scale, lane);     // T2K [q][b=x][c=y][l]
+        pack_store<MODE>(T2KT + (((size_t)q * v + (y0 + yy)) * vp + x) * ok, ch, xv, scale, lane);    // T2KT[q][b=y][c=x][l]
     }
 }
 
@@ -239,15 +244,14 @@ template <int MODE>
 __global__ void __launch_bounds__(256)
 pack_t2a_kernel(const double* __restrict__ t2, size_t rows, int v, int vk, uint32_t* __restrict__ T2A,
                 const float* __restrict__ sc) {
-    constexpr int CW = MODE ? 64 : 32;
     const double scale = pack_scale<MODE>(sc, 1);
-    const int lane = threadIdx.x & 31, nch = vk / CW;
+    const int lane = threadIdx.x & 31, nch = pack_chunks<MODE>(vk);
     const size_t nw = rows * nch;
     for (size_t w = blockIdx.x * (size_t)8 + (threadIdx.x >> 5); w < nw; w += (size_t)gridDim.x * 8) {
         const size_t row = w / nch;
         const int ch = (int)(w % nch), d = ch * 32 + lane;
         const double x = d < v ? t2[row * v + d] : 0.0;
-        pack_store<MODE>(T2A + row * vk + (size_t)ch * CW, x, scale, lane);
+        pack_store<MODE>(T2A + row * vk, ch, x, scale, lane);
     }
 }
 
@@ -256,16 +260,15 @@ template <int MODE>
 __global__ void __launch_bounds__(256)
 pack_ota_kernel(const double* __restrict__ ovoo, int v, int o, int ok, uint32_t* __restrict__ OtA,
                 const float* __restrict__ sc) {
-    constexpr int CW = MODE ? 64 : 32;
     const double scale = pack_scale<MODE>(sc, 0);
-    const int lane = threadIdx.x & 31, nch = ok / CW;
+    const int lane = threadIdx.x & 31, nch = pack_chunks<MODE>(ok);
     const size_t nw = (size_t)o * o * v * nch;
     for (size_t w = blockIdx.x * (size_t)8 + (threadIdx.x >> 5); w < nw; w += (size_t)gridDim.x * 8) {
         const size_t row = w / nch;                        // (r, p, a)
         const int ch = (int)(w % nch), l = ch * 32 + lane;
         const int a = (int)(row % v), p = (int)((row / v) % o), r = (int)(row / ((size_t)v * o));
         const double x = l < o ? -ovoo[(((size_t)p * v + a) * o + l) * o + r] : 0.0;
-        pack_store<MODE>(OtA + row * ok + (size_t)ch * CW, x, scale, lane);
+        pack_store<MODE>(OtA + row * ok, ch, x, scale, lane);
     }
 }
 

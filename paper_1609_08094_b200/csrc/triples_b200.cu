@@ -372,7 +372,7 @@ int pack_xk(const Plan& P, const double* src, int ro, int sp, int slot0, const O
     auto kern = P.prec == TRIPLES_EMU64 ? pack_xk_kernel<1> : pack_xk_kernel<0>;
     CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, PKX_SMEM));
     const size_t S = (size_t)P.v * P.v * ro;
-    dim3 grid((unsigned)((S + PKX_SPAN - 1) / PKX_SPAN), P.vk / P.kwords);
+    dim3 grid((unsigned)((S + PKX_SPAN - 1) / PKX_SPAN), P.kchunks_v);
     kern<<<grid, 256, PKX_SMEM, st>>>(src, P.v, P.vp, P.vk, ro, sp, slot0, (uint32_t*)op.x, (uint32_t*)op.xt, op.scales);
     CU_TRY(cudaGetLastError());
     ++g_launches;
