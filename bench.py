@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """Benchmark of the B200 closed-shell (T) energy path (arXiv:1609.08094 section 2.2).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config medium] [--precision fp64|mixed]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config medium] [--precision fp64|mixed|emu64]
     python bench.py --impl reference ...          # the CPU oracle, timed on the host cores
 
 A "step" is one pass of the whole hot path -- repack, every contraction batch, every fused reduction batch,
@@ -13,7 +13,8 @@ coinciding contractions of i=j / j=k tasks computed once) and is the figure to h
 
 The default line (medium, FP64) also carries: the mixed-precision path on the same workload (`mixed_path`), the
 RI-direct and out-of-core variants (`ri_direct`, `streamed`), and short legs on the two largest single-GPU
-configs (`legs.large`: FP64 + mixed + streamed, `legs.largest`: mixed), each with its own roofline fractions
+configs (`legs.large`: FP64 + mixed + emulated FP64 + streamed, `legs.largest`: mixed + emulated FP64; `emu64_path`:
+FP64-class results from the INT8 tensor cores on the default workload), each with its own roofline fractions
 and its parity against the stored oracle values of tests/golden/.  --no-legs / --no-variants skip them.
 
 Multi-GPU: north_star builds a single-GPU path ("replicas only"): --gpus N runs N
@@ -437,6 +438,7 @@ def main():
             host = {k: dev[k].cpu().numpy() for k in NAMES}
     dargs = [dev[k] for k in NAMES]
     mixed_leg = prec == tb.FP64 and world == 1 and not args.no_mixed_leg and args.config in ("tiny", "small", "medium")
+    emu_leg = mixed_leg
     ws_bytes = tb.triples_workspace_bytes_host(o, v, prec)
     if mixed_leg:
         ws_bytes = max(ws_bytes, tb.triples_workspace_bytes(o, v, tb.MIXED), tb.triples_workspace_bytes(o, v, tb.EMU64))
@@ -532,6 +534,15 @@ def main():
             "note": "tolerance 1e-5 on E(T); E5 is 1e-7..1e-4 of E4 with the generator's t1 ~ N(0,1e-3^2) and a sum of both "
                     "signs, so its deviation is given on the scale of E4 (tests pin E5 with t1 ~ N(0,1))"}
 
+    # ---- FP64-class results from the INT8 tensor cores: same workload, FP64 tolerance
+    emu = None
+    if emu_leg:
+        emu, Ee = precision_leg(tb, torch, args.config, tb.EMU64, o, v, dargs, ws, stream, args.steps, 1, peaks, peak_kind,
+                                fp64_peak, index)
+        emu["rel_dev_from_fp64"] = {"E_T": abs(Ee[0] - E[0]) / abs(E[0]), "E4": abs(Ee[1] - E[1]) / abs(E[1]),
+                                    "E5": abs(Ee[2] - E[2]) / abs(E[2])}
+        emu["speedup_over_fp64_path"] = (sec / args.steps) / emu["s_per_ET"]
+
     # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample (rank 0, N=1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -580,7 +591,7 @@ def main():
         del dargs, dev, ws, et
         host = None
         import gc
-        for cfg, precs in (("large", (tb.FP64, tb.MIXED)), ("largest", (tb.MIXED,))):
+        for cfg, precs in (("large", (tb.FP64, tb.MIXED, tb.EMU64)), ("largest", (tb.MIXED, tb.EMU64))):
             gc.collect()
             torch.cuda.empty_cache()
             lo, lv, lnaux = synth.CONFIGS[cfg]
@@ -591,11 +602,12 @@ def main():
             largs = [d[k] for k in NAMES]
             lws = torch.empty(max(tb.triples_workspace_bytes(lo, lv, p) for p in precs), dtype=torch.uint8, device="cuda")
             lindex = {t: n for n, t in enumerate(synth.triplet_list(lo))}
-            leg = {"workload": workload_name(cfg, "+".join("fp64" if p == tb.FP64 else "mixed" for p in precs), lo, lv, lnaux),
+            pname = {tb.FP64: "fp64", tb.MIXED: "mixed", tb.EMU64: "emu64"}
+            leg = {"workload": workload_name(cfg, "+".join(pname[p] for p in precs), lo, lv, lnaux),
                    "input_generation_s": gen_s}
             for p in precs:
-                key = "fp64" if p == tb.FP64 else "mixed"
-                leg[key], El = precision_leg(tb, torch, cfg, p, lo, lv, largs, lws, stream, 1 if p == tb.FP64 else 2, 1,
+                key = pname[p]
+                leg[key], El = precision_leg(tb, torch, cfg, p, lo, lv, largs, lws, stream, 2 if p == tb.MIXED else 1, 1,
                                              peaks, peak_kind, fp64_peak, lindex)
                 if cfg == "large" and p == tb.FP64 and not args.no_variants:
                     del lws
@@ -628,6 +640,8 @@ def main():
         }
         if mixed is not None:
             line["mixed_path"] = mixed
+        if emu is not None:
+            line["emu64_path"] = emu
         if ri is not None:
             line["ri_direct"] = ri
         if streamed is not None:

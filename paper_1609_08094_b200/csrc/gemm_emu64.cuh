@@ -4,16 +4,19 @@
 // the 37 TFLOP/s FP64 tensor peak) and the FP16-split path (gemm_f16split.cuh).
 //
 // Ozaki-style error-free slicing with ONE power-of-two scale per tensor class (as on the mixed path): every operand
-// is the 42-bit fixed-point integer xi = rint(x 2^(s+26)) = sum_i d_i 128^(5-i), six balanced base-128 digits
-// d_i in [-64, 63] (prepare.cuh pack_emu_store).  Then
-//     sum_k xi_k yi_k = sum_{i,j} 128^(10-i-j) S_ij,   S_ij = sum_k d_i(x_k) d_j(y_k)   (an exact int8 x int8 -> int32 GEMM)
-// and the pairs of one LEVEL L = i + j share a weight, so they accumulate in ONE int32 TMEM accumulator: (L+1) K 64^2
-// < 2^31 for K <= 87000.  Levels L <= 5 are kept (21 digit products per 32 K elements); the dropped levels are below
-// 2^-38 of (class maximum)^2 per term, of the order of the 2^-40 quantisation of the operands themselves.  Integer
-// accumulation is exact, so -- unlike the FP16-split kernel -- a whole work item (all four K segments) accumulates in
-// TMEM and is read out once: S_L -> double, W = sum_L S_L c_L with the exact powers of two
-// c_L = 2^(7(10-L) - (sg+st) - 52); six FMAs per element, rounding ~1e-16.  (A first version with seven digits and
-// levels <= 6 -- 28 products, BN = 64 -- measured 2e-14 per-triplet parity and 73 TFLOP/s at medium.)
+// is the 47-bit fixed-point integer xi = rint(x 2^(s+32)) = sum_i d_i 256^(5-i), six balanced base-256 digits
+// d_i in [-128, 127] (prepare.cuh pack_emu_store).  Then
+//     sum_k xi_k yi_k = sum_{i,j} 256^(10-i-j) S_ij,   S_ij = sum_k d_i(x_k) d_j(y_k)   (an exact s8 x s8 -> s32 GEMM)
+// and the pairs of one LEVEL L = i + j share a weight, so they accumulate in ONE int32 TMEM accumulator: (L+1) K 128^2
+// < 2^31 for K <= 21000.  Levels L <= 5 are kept (21 digit products per 32 K elements).  What is dropped: for the x
+// digit i the y digits below 5-i, i.e. y rounded to nearest (balanced digits) at the unit of its digit 5-i -- per term
+// d_i 256^(5-i) * (<= 0.5 * 256^i) <= 2^46, against products of up to 2^92: ~2^-50 of (class maximum)^2 per term,
+// below the 2^-46 quantisation of the operands themselves.  Integer accumulation is exact, so -- unlike the
+// FP16-split kernel -- a whole work item (all four K segments) accumulates in TMEM and is read out once:
+// S_L -> double, W = sum_L S_L c_L with the exact powers of two c_L = 2^(8(10-L) - (sg+st) - 64); six FMAs per
+// element, rounding ~1e-16.  Measured: W within 1e-13 of the oracle on the scale of W.  (Earlier digit choices, same
+// cost per product: 7 digits base 128, levels <= 6, 28 products, BN = 64: 73 TFLOP/s, W within 1e-12; 6 digits base
+// 128, levels <= 5: W only within 1e-10 -- the amplitudes' dynamic range eats the 7-bit digits.)
 //
 // Same G job, tiling and roles as gemm_f16split.cuh (transposed: the (b,c) index is the MMA's M dimension, CTA pairs,
 // 128 TMEM lanes per CTA), with BN = 80 a-columns per tile: six level accumulators of 80 columns = 480 of the 512
@@ -182,7 +185,7 @@ gemm_emu64_kernel(const __grid_constant__ EmuMaps maps, const GemmJob* __restric
         constexpr int HC = EM_BN / 2;                       // columns per warp
         const int half = (warp - EM_ACC_WARP0) >> 2;        // columns [40*half, 40*half + 40) of every level
         const uint32_t ltempty = mapa_u32(smem_u32(&tempty[0]), 0);
-        const int sexp = reinterpret_cast<const int*>(scales)[12] + reinterpret_cast<const int*>(scales)[13] + 52;
+        const int sexp = reinterpret_cast<const int*>(scales)[12] + reinterpret_cast<const int*>(scales)[13] + 64;
         uint32_t item = 0;
         for (long long w = cid; w < nitems; w += ncl, ++item) {
             int jb, rem;
@@ -195,7 +198,7 @@ gemm_emu64_kernel(const __grid_constant__ EmuMaps maps, const GemmJob* __restric
             tc_fence_after_sync();
 #pragma unroll
             for (int L = 0; L < EM_LEVELS; ++L) {
-                const double cL = ldexp(1.0, 7 * (10 - L) - sexp);       // exact power of two
+                const double cL = ldexp(1.0, 8 * (10 - L) - sexp);       // exact power of two
                 const uint32_t taddr = tmem_base + (uint32_t)L * EM_BN + half * HC + ((uint32_t)(wq * 32) << 16);
 #pragma unroll
                 for (int c0 = 0; c0 < 32; c0 += 16) {

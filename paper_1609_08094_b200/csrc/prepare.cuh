@@ -131,13 +131,13 @@ __device__ __forceinline__ void pack_split_store(uint32_t* __restrict__ row, flo
     row[(lane >> 1) + (odd ? 16 : 0)] = odd ? (got | (mine << 16)) : (mine | (got << 16));
 }
 
-// Emulated-FP64 path (gemm_emu64.cuh): the scaled value is rounded to a 42-bit fixed-point integer
-// xi = rint(x * 2^(s + 26)) (|xi| < 2^40: the class maximum sits in [2^39, 2^40)) and cut into six balanced base-128
-// digits d_0 (most significant) .. d_5 in [-64, 63], xi = sum_i d_i 128^(5-i).  K is walked in chunks of 64; per
+// Emulated-FP64 path (gemm_emu64.cuh): the scaled value is rounded to a 47-bit fixed-point integer
+// xi = rint(x * 2^(s + 32)) (|xi| < 2^46: the class maximum sits in [2^45, 2^46)) and cut into six balanced base-256
+// digits d_0 (most significant, |d_0| <= 64) .. d_5 in [-128, 127], xi = sum_i d_i 256^(5-i).  K is walked in chunks of 64; per
 // operand row and chunk THREE 128-byte rows (96 words): row p holds digit 2p of the 64 K elements in bytes 0..63 and
 // digit 2p+1 in bytes 64..127 -- 6 bytes per element, no padding.  The 32 lanes of a warp hold 32 consecutive K
 // elements = half h of a chunk.
-constexpr int EMU_SHIFT = 26;
+constexpr int EMU_SHIFT = 32;
 constexpr int EMU_DIGITS = 6;
 constexpr int EMU_CHUNK_WORDS = 96;
 __device__ __forceinline__ void pack_emu_store(uint32_t* __restrict__ chunk, int h, double x, int lane) {
@@ -145,10 +145,10 @@ __device__ __forceinline__ void pack_emu_store(uint32_t* __restrict__ chunk, int
     int8_t d[EMU_DIGITS];
 #pragma unroll
     for (int i = EMU_DIGITS - 1; i >= 0; --i) {
-        int r = (int)(xi & 127);
-        if (r >= 64) r -= 128;
+        int r = (int)(xi & 255);
+        if (r >= 128) r -= 256;
         d[i] = (int8_t)r;
-        xi = (xi - r) >> 7;
+        xi = (xi - r) >> 8;
     }
     int8_t* b = reinterpret_cast<int8_t*>(chunk);
 #pragma unroll
