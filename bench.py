@@ -40,7 +40,7 @@ if ROOT not in sys.path:
 
 NAMES = ("eps_o", "eps_v", "t1", "t2", "vvvo", "ovoo", "ovov")
 MIXED_DTYPE = "fp16 split x = h + l (f32 accumulate), f64 reduction"
-EMU_DTYPE = "f64 emulated: 7 base-128 int8 digits per operand, 28 exact s8 x s8 -> s32 products, f64 recombination and reduction"
+EMU_DTYPE = "f64 emulated: 6 base-256 int8 digits per operand, 21 exact s8 x s8 -> s32 products, f64 recombination and reduction"
 GOLDEN_OF = {"small": "small_full", "medium": "medium_full", "large": "large_sample", "largest": "largest_sample"}
 
 
@@ -253,10 +253,10 @@ def rooflines(tb, prec, prof, peaks, peak_kind, fp64_peak, traffic):
         peak_note = fp64_peak["note"]
     elif prec == tb.EMU64:
         kernel = "gemm_emu64_kernel"
-        peak = peaks["bf16_tflops_sustained"] * 2.0 / 28.0
+        peak = peaks["bf16_tflops_sustained"] * 2.0 / 21.0
         peak_note = (f"INT8 dense tensor rate = 2 x bf16 sustained cuBLAS ({peak_kind}, MEASURED_PEAKS.json; the guide's nominal "
-                     "int8:bf16 ratio) / 28: every FP64-class product costs 28 int8 digit products (levels <= 6 of 7 x 7 "
-                     "digits). achieved = ALGORITHMIC flops; vs_native_fp64_peak = achieved / the DMMA peak measured in "
+                     "int8:bf16 ratio) / 21: every FP64-class product costs 21 int8 digit products (levels <= 5 of 6 x 6 "
+                     "base-256 digits). achieved = ALGORITHMIC flops; vs_native_fp64_peak = achieved / the DMMA peak measured in "
                      "this run (> 1: faster than the native FP64 tensor pipe can go)")
     else:
         kernel = "gemm_f16split_kernel"
@@ -273,7 +273,7 @@ def rooflines(tb, prec, prof, peaks, peak_kind, fp64_peak, traffic):
         roof["tensor_pipe_tf32_equiv"] = 1.5 * gemm_tflops
         roof["frac_tensor_pipe"] = 1.5 * gemm_tflops / peak
     if prec == tb.EMU64:
-        roof["tensor_pipe_int8"] = 28.0 * gemm_tflops
+        roof["tensor_pipe_int8"] = 21.0 * gemm_tflops
         roof["vs_native_fp64_peak"] = gemm_tflops / fp64_peak["tflops"]
     nr = max(prof["reduction_launches"], 1)
     red = {"bound": "hbm", "kernel": "reduce_kernel<float>" if prec == tb.MIXED else "reduce_kernel<double>",

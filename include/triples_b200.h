@@ -40,12 +40,13 @@
  *                x = h + l in FP16, h*h' + h*l' + l*h' on tcgen05 with FP32 accumulation, W stored FP32:
  *                W within 1e-6 of FP64 on the scale of W); Vd, D, the energy reduction and sums in FP64.
  *                TRIPLES_EMU64 = FP64-class contractions emulated on the INT8 tensor cores (a
- *                third point of the paper's precision study, L125, L156-L158): operands as 49-bit fixed point relative
- *                to the largest element of their tensor class, cut into seven base-128 digits; the digit products
- *                are exact integer GEMMs (tcgen05 kind::i8), recombined in FP64; W stored FP64, everything else as
- *                TRIPLES_FP64.  Same tolerance as TRIPLES_FP64 for inputs whose elements span < ~2^13 within a
- *                tensor class at the accuracy that matters.  Resident entry points only (triples_energy, _host,
- *                _sharded, _subset, _w_block); the streamed / RI entries return TRIPLES_EINVAL.
+ *                third point of the paper's precision study, L125, L156-L158): operands as 47-bit fixed point relative
+ *                to the largest element of their tensor class (integrals / amplitudes), cut into six base-256
+ *                digits; the digit products are exact integer GEMMs (tcgen05 kind::i8), recombined in FP64; W stored
+ *                FP64, everything else as TRIPLES_FP64.  Tolerance: the FP64 one.  Error model: ABSOLUTE, ~2^-46 of
+ *                the class maximum per operand element (an element 2^-n below the maximum keeps 47-n bits).
+ *                Resident entry points only (triples_energy, _host, _sharded, _subset, _w_block); the streamed / RI
+ *                entries return TRIPLES_EINVAL for it.
  */
 #ifndef TRIPLES_B200_H
 #define TRIPLES_B200_H
