@@ -356,7 +356,7 @@ def streamed_leg(tb, torch, o, v, d, prec, stream, nslots, win, resident_sec, E_
     for k in range(o):                                  # generator-side reshuffle to the slice-major layout
         host[k].copy_(vv[:, :, :, k])
     torch.cuda.synchronize()
-    absmax = float(vv.abs().max().item()) if prec == tb.MIXED else 0.0
+    absmax = float(vv.abs().max().item()) if prec != tb.FP64 else 0.0
     nbytes = tb.triples_workspace_bytes_streamed(o, v, prec, nslots, win)
     slots, w = tb.triples_cache_slots(o, v, 0, prec, 1, nbytes)
     ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
@@ -609,10 +609,10 @@ def main():
                 key = pname[p]
                 leg[key], El = precision_leg(tb, torch, cfg, p, lo, lv, largs, lws, stream, 2 if p == tb.MIXED else 1, 1,
                                              peaks, peak_kind, fp64_peak, lindex)
-                if cfg == "large" and p == tb.FP64 and not args.no_variants:
+                if cfg == "large" and p in (tb.FP64, tb.EMU64) and not args.no_variants:
                     del lws
                     torch.cuda.empty_cache()
-                    leg["streamed_fp64"] = streamed_leg(tb, torch, lo, lv, d, p, stream, 16, 2, leg[key]["s_per_ET"], El)
+                    leg["streamed_" + key] = streamed_leg(tb, torch, lo, lv, d, p, stream, 16, 2, leg[key]["s_per_ET"], El)
                     lws = torch.empty(max(tb.triples_workspace_bytes(lo, lv, q) for q in precs), dtype=torch.uint8,
                                       device="cuda")
             legs[cfg] = leg

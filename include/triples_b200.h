@@ -45,8 +45,7 @@
  *                digits; the digit products are exact integer GEMMs (tcgen05 kind::i8), recombined in FP64; W stored
  *                FP64, everything else as TRIPLES_FP64.  Tolerance: the FP64 one.  Error model: ABSOLUTE, ~2^-46 of
  *                the class maximum per operand element (an element 2^-n below the maximum keeps 47-n bits).
- *                Resident entry points only (triples_energy, _host, _sharded, _subset, _w_block); the streamed / RI
- *                entries return TRIPLES_EINVAL for it.
+ *                Every entry point takes it (streamed / RI slices are staged in FP64 and digitised on the device).
  */
 #ifndef TRIPLES_B200_H
 #define TRIPLES_B200_H

@@ -118,7 +118,6 @@ inline int min_slots(int o, int win, int mode) {
 inline bool make_plan(int o, int v, int prec, Plan& P, int mode = SLICES_RESIDENT, int nslots = 0, int naux = 0,
                       int win_cap = 0) {
     if (o < 1 || v < 1 || o > kMaxOcc || v > kMaxVirt || (prec < 0 || prec > 2)) return false;
-    if (prec == 2 && mode != SLICES_RESIDENT) return false;     // emulated FP64: resident slices only
     if (mode < 0 || mode > 2 || nslots < 0 || (mode == SLICES_RI && naux < 1)) return false;
     P = Plan();
     P.o = o; P.v = v; P.prec = prec; P.mode = mode;
@@ -187,8 +186,8 @@ inline bool make_plan(int o, int v, int prec, Plan& P, int mode = SLICES_RESIDEN
         P.nslots = nslots < lo ? lo : (nslots > o ? o : nslots);
     }
     P.n_x = (size_t)P.nslots * P.n_slice;
-    if (prec == 1 && mode == SLICES_STREAMED) P.nstage = 2 * min_slots(o, win, SLICES_RI);
-    if (prec == 1 && mode == SLICES_RI) P.nstage = 1;
+    if (prec != 0 && mode == SLICES_STREAMED) P.nstage = 2 * min_slots(o, win, SLICES_RI);   // packed paths: FP64 staging
+    if (prec != 0 && mode == SLICES_RI) P.nstage = 1;
     if (mode == SLICES_RI) {   // X_r[(d,b)][c] = sum_Q Bt[(d,b)][Q] Bo[r][Q][c]: M = v^2, N = v, K = naux
         P.naux = naux;
         P.nauxp = (naux + 1) & ~1;

@@ -11,7 +11,7 @@ from paper_1609_08094_b200 import synth
 
 pytestmark = pytest.mark.gpu
 
-TOL = {tb.FP64: 1e-10, tb.MIXED: 1e-5}
+TOL = {tb.FP64: 1e-10, tb.MIXED: 1e-5, tb.EMU64: 1e-10}
 STREAMED, RI = 1, 2
 
 
@@ -37,7 +37,7 @@ def slice_major_host(inp):
     return t, t.numpy()
 
 
-@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED], ids=["fp64", "mixed"])
+@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED, tb.EMU64], ids=["fp64", "mixed", "emu64"])
 @pytest.mark.parametrize("o,v,naux,win,extra", [(6, 24, 40, 1, 0), (7, 33, 40, 1, 1), (9, 40, 50, 2, 0), (14, 64, 70, 2, 2),
                                                 (5, 17, 30, 0, 0)])
 def test_streamed_is_bitwise_the_resident_run(o, v, naux, win, extra, prec):
@@ -79,7 +79,7 @@ def test_streamed_profile_counts_slices_and_bytes():
     assert p["slices_loaded"] == len(loads) and p["h2d_bytes"] == len(loads) * 8 * v ** 3
 
 
-@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED], ids=["fp64", "mixed"])
+@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED, tb.EMU64], ids=["fp64", "mixed", "emu64"])
 @pytest.mark.parametrize("o,v,naux,slots", [(3, 5, 9, 0), (6, 24, 37, 0), (8, 40, 120, 0), (7, 33, 50, 7), (9, 48, 130, 4),
                                             (5, 130, 40, 0)])
 def test_ri_direct_matches_the_oracle(o, v, naux, slots, prec):
@@ -108,7 +108,7 @@ def test_ri_direct_matches_the_oracle(o, v, naux, slots, prec):
         assert abs(E[0] - Er[0]) <= 1e-12 * abs(Er[0])
 
 
-@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED], ids=["fp64", "mixed"])
+@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED, tb.EMU64], ids=["fp64", "mixed", "emu64"])
 @pytest.mark.parametrize("o,v,naux,nshards", [(6, 24, 40, 2), (9, 40, 50, 3), (8, 40, 120, 8), (3, 9, 12, 5)])
 def test_sharded_partials_add_up_to_the_full_run(o, v, naux, nshards, prec):
     inp = synth.make_inputs(o, v, naux, seed=8, t1_sigma=0.2)
