@@ -196,24 +196,29 @@ gemm_emu64_kernel(const __grid_constant__ EmuMaps maps, const GemmJob* __restric
             for (int j = 0; j < HC; ++j) acc[j] = 0.0;
             mbar_wait(&tfull[0], item & 1);
             tc_fence_after_sync();
+            // Read-out, software-pipelined: five segments of 8 columns per level; the tcgen05.ld of segment s+1 is in
+            // flight while segment s is converted, so the TMEM read port (64 B/clk), not the conversions, sets the
+            // length of the serial section.  int32 -> double without the XU pipe: the bits 0x43300000'80000000 ^ x
+            // are the double 2^52 + 2^31 + x (exact), one DADD removes the offset, one DFMA applies the level weight.
+            {
+                const uint32_t tlane = tmem_base + half * HC + ((uint32_t)(wq * 32) << 16);
+                constexpr int NSEG = EM_LEVELS * (HC / 8);
+                uint32_t rg[2][8];
+                tmem_ld_32x32b_x8(tlane, rg[0]);
 #pragma unroll
-            for (int L = 0; L < EM_LEVELS; ++L) {
-                const double cL = ldexp(1.0, 8 * (10 - L) - sexp);       // exact power of two
-                const uint32_t taddr = tmem_base + (uint32_t)L * EM_BN + half * HC + ((uint32_t)(wq * 32) << 16);
-#pragma unroll
-                for (int c0 = 0; c0 < 32; c0 += 16) {
-                    uint32_t rg[16];
-                    tmem_ld_32x32b_x16(taddr + c0, rg);
+                for (int sgm = 0; sgm < NSEG; ++sgm) {
+                    const int L = sgm / (HC / 8), c0 = (sgm % (HC / 8)) * 8;
                     tmem_ld_wait();
+                    if (sgm + 1 < NSEG) {
+                        const int Ln = (sgm + 1) / (HC / 8), cn = ((sgm + 1) % (HC / 8)) * 8;
+                        tmem_ld_32x32b_x8(tlane + (uint32_t)Ln * EM_BN + cn, rg[(sgm + 1) & 1]);
+                    }
+                    const double cL = ldexp(1.0, 8 * (10 - L) - sexp);       // exact power of two
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) acc[c0 + j] = fma((double)(int)rg[j], cL, acc[c0 + j]);
-                }
-                {
-                    uint32_t rg[8];
-                    tmem_ld_32x32b_x8(taddr + 32, rg);
-                    tmem_ld_wait();
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) acc[32 + j] = fma((double)(int)rg[j], cL, acc[32 + j]);
+                    for (int j = 0; j < 8; ++j) {
+                        const double dv = __hiloint2double(0x43300000, (int)(rg[sgm & 1][j] ^ 0x80000000u)) - 4503601774854144.0;
+                        acc[c0 + j] = fma(dv, cL, acc[c0 + j]);
+                    }
                 }
             }
             tc_fence_before_sync();

@@ -374,6 +374,32 @@ def test_mixed_path_magnitudes_far_from_one(lam, mu):
     assert abs(E[2] - Eo[2]) <= TOL[tb.MIXED] * max(abs(Eo[2]), 1e-3 * abs(Eo[1]))
 
 
+@pytest.mark.parametrize("lam,mu", [(1.0, 1.0), (3e-9, 2e5), (4e6, 7e-8), (1e-20, 1e12)])
+def test_emu64_path_magnitudes_far_from_one(lam, mu):
+    """The fixed-point digits are taken relative to a power-of-two scale per tensor class: the overall magnitude of
+    the amplitudes / integrals must not matter (t2 -> lam t2, integrals -> mu g)."""
+    inp = synth.make_inputs(5, 41, 60, seed=6, t1_sigma=0.3)
+    s = synth.TriplesInputs(inp.nocc, inp.nvirt, inp.eps_o, inp.eps_v, inp.t1, inp.t2 * lam, inp.vvvo * mu,
+                            inp.ovoo * mu, inp.ovov * mu)
+    E = gpu_energy(s, prec=tb.EMU64)
+    Eo = oracle.energy_restricted(s.nocc, s.nvirt, *s.arrays())
+    assert rel(E[0], Eo[0]) <= TOL[tb.EMU64] and rel(E[1], Eo[1]) <= TOL[tb.EMU64]
+    assert abs(E[2] - Eo[2]) <= TOL[tb.EMU64] * max(abs(Eo[2]), 1e-3 * abs(Eo[1]))
+
+
+def test_emu64_path_wide_dynamic_range_amplitudes():
+    """Amplitudes spread over 12 orders of magnitude (row-wise factors): the error model of the emulated path is
+    absolute per tensor class (2^-46 of the class maximum per element), so E(T) -- dominated by the large
+    amplitudes -- keeps the FP64 tolerance although the smallest amplitudes keep only a few bits."""
+    inp = synth.make_inputs(5, 41, 60, seed=7, t1_sigma=0.0)
+    f = np.logspace(0, -6, inp.nvirt)
+    t2 = inp.t2 * f[None, None, :, None] * f[None, None, None, :]
+    s = synth.TriplesInputs(inp.nocc, inp.nvirt, inp.eps_o, inp.eps_v, inp.t1, t2, inp.vvvo, inp.ovoo, inp.ovov)
+    E = gpu_energy(s, prec=tb.EMU64)
+    Eo = oracle.energy_restricted(s.nocc, s.nvirt, *s.arrays())
+    assert rel(E[0], Eo[0]) <= TOL[tb.EMU64]
+
+
 def test_mixed_path_wide_dynamic_range_amplitudes():
     """Amplitudes spread over 12 orders of magnitude (row-wise factors): elements far below the tensor maximum fall to
     the split's absolute floor (2^-39 of the maximum), which must not hurt the energy."""
