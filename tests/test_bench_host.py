@@ -107,3 +107,22 @@ def test_reference_arm_times_the_oracle_and_prints_one_json_line():
 def test_reference_arm_other_ranks_exit_quietly():
     res = _run_reference({"RANK": "1", "WORLD_SIZE": "2", "LOCAL_RANK": "1"})
     assert res.returncode == 0 and res.stdout.strip() == ""
+
+
+def test_parity_vs_golden_compares_the_stored_oracle_values():
+    """bench.py's parity figure: the run's per-triplet energies against tests/golden/ (no oracle run, no GPU)."""
+    import numpy as np
+    g = bench.load_golden("small")
+    o = g["nocc"]
+    trip = [(i, j, k) for i in range(o) for j in range(i, o) for k in range(j, o)]
+    index = {t: n for n, t in enumerate(trip)}
+    et = np.zeros((len(trip), 3))
+    for t, e in zip(g["triplets_ijk"], g["energies"]):
+        et[index[tuple(t)]] = e
+    exact = bench.parity_vs_golden("small", et, index, 1e-10)
+    assert exact["ok"] and exact["max_rel_err"] == 0.0 and exact["triplets_compared"] == len(trip) - o
+    n = index[(0, 1, 2)]
+    et[n, 0] *= 1 + 3e-9
+    off = bench.parity_vs_golden("small", et, index, 1e-10)
+    assert not off["ok"] and 2e-9 < off["max_rel_err"] < 4e-9
+    assert bench.parity_vs_golden("tiny", et, index, 1e-10) is None          # no stored file for that config name
