@@ -37,8 +37,8 @@ struct alignas(64) EmuMaps {
 };
 
 constexpr int EM_BM = 128;            // (b,c) rows per CTA tile = TMEM lanes
-constexpr int EM_BN = 80;             // a-columns per tile
-constexpr int EM_NPAD = EM_BN / 2;    // N-side rows a CTA stages
+// a-columns per tile: template parameter BN in {80, 64, 48} (six level accumulators x BN <= 512 TMEM columns; plan.h
+// picks the one that wastes the least MMA time on padded columns, charging the smaller tiles their extra feed)
 constexpr int EM_DIGITS = 6;
 constexpr int EM_LEVELS = 6;          // levels 0..5 kept
 constexpr int EM_BK = 64;             // K elements per chunk
@@ -48,15 +48,19 @@ constexpr int EM_THREADS = 384;
 constexpr int EM_ACC_WARP0 = 4;
 constexpr int EM_TMEM_COLS = 512;
 constexpr int EM_STAGES = 3;
-constexpr int EM_TILE_BYTES = EM_ROWS * (EM_BM + EM_NPAD) * 128;      // 63 KB: [M row 0..2][N row 0..2]
+__host__ __device__ constexpr int em_tile_bytes(int bn) { return EM_ROWS * (EM_BM + bn / 2) * 128; }   // [M row 0..2][N row 0..2]
 constexpr int EM_MAX_JOBS = 192;
 constexpr int EM_TAIL_BYTES = 2048 + EM_MAX_JOBS * 48;
-constexpr int EM_SMEM_BYTES = EM_STAGES * EM_TILE_BYTES + EM_TAIL_BYTES;
+__host__ __device__ constexpr int em_smem_bytes(int bn) { return EM_STAGES * em_tile_bytes(bn) + EM_TAIL_BYTES; }
 
+template <int EM_BN>
 __global__ void __launch_bounds__(EM_THREADS, 1)
 gemm_emu64_kernel(const __grid_constant__ EmuMaps maps, const GemmJob* __restrict__ gjobs, int njobs, int v, int vp, int o,
                   int mtiles, int ntiles, const float* __restrict__ scales) {
     constexpr int cs = 2;
+    constexpr int EM_NPAD = EM_BN / 2;                     // N-side rows a CTA stages
+    constexpr int EM_TILE_BYTES = em_tile_bytes(EM_BN);
+    static_assert(EM_LEVELS * EM_BN <= EM_TMEM_COLS && EM_NPAD % 8 == 0, "level accumulators fit TMEM; whole swizzle atoms");
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* smem_tail = smem + EM_STAGES * EM_TILE_BYTES;

@@ -154,8 +154,16 @@ inline bool make_plan(int o, int v, int prec, Plan& P, int mode = SLICES_RESIDEN
         } else {               // emulated FP64: 96 words (three 128-byte rows of digit pairs) per 64-wide K chunk
             P.vk = (v + 63) / 64 * 96; P.ok = (o + 63) / 64 * 96;
             P.kchunks_v = P.vk / 96 * 2; P.kchunks_o = P.ok / 96 * 2;
-            P.tf_bn = 80;
-            P.tf_ntiles = (v + 79) / 80;
+            // tile width 80 / 64 / 48 columns: MMA time goes with the padded column count; the narrower tiles re-stage
+            // the M-side rows more often (bytes per MMA clock 38 / 46 / 58 against the ~42 an SM can take in)
+            const int bnc[3] = {80, 64, 48};
+            const double feed[3] = {1.0, 1.09, 1.38};
+            double bestc = -1.0;
+            for (int c = 0; c < 3; ++c) {
+                const double cost = (double)((v + bnc[c] - 1) / bnc[c] * bnc[c]) * feed[c];
+                if (bestc < 0 || cost < bestc) { bestc = cost; P.tf_bn = bnc[c]; }
+            }
+            P.tf_ntiles = (v + P.tf_bn - 1) / P.tf_bn;
         }
         P.tf_mtiles = (int)((N + 127) / 128);
         // CTA pairs (cta_group::2): a pair owns two consecutive m-tiles, each CTA stages half of the N-side rows

@@ -218,8 +218,8 @@ int build_maps_emu(const Plan& P, const Operands& op, EmuMaps* maps) {
     if ((rc = make_map3(&maps->xkt, dt, 4, op.xt, vk, NR, ns, vk, NR * vk, 32, EM_BM, 1))) return rc;
     if ((rc = make_map3(&maps->t2k, dt, 4, op.t2k, ok, NR, o, ok, NR * ok, 32, EM_BM, 1))) return rc;
     if ((rc = make_map3(&maps->t2kt, dt, 4, op.t2kt, ok, NR, o, ok, NR * ok, 32, EM_BM, 1))) return rc;
-    if ((rc = make_map3(&maps->t2a, dt, 4, op.t2, vk, v, o * o, vk, v * vk, 32, EM_NPAD, 1))) return rc;
-    if ((rc = make_map3(&maps->ota, dt, 4, op.ot, ok, v, o * o, ok, v * ok, 32, EM_NPAD, 1))) return rc;
+    if ((rc = make_map3(&maps->t2a, dt, 4, op.t2, vk, v, o * o, vk, v * vk, 32, P.tf_npad, 1))) return rc;
+    if ((rc = make_map3(&maps->ota, dt, 4, op.ot, ok, v, o * o, ok, v * ok, 32, P.tf_npad, 1))) return rc;
     return TRIPLES_OK;
 }
 
@@ -247,7 +247,7 @@ int max_pair_clusters(K kern, int which, cudaLaunchConfig_t cfg, int cs, int* ou
     int dev = 0;
     CU_TRY(cudaGetDevice(&dev));
     std::lock_guard<std::mutex> lk(mu);
-    const auto key = std::make_pair(dev * 2 + which, cfg.dynamicSmemBytes);
+    const auto key = std::make_pair(dev * 8 + which, cfg.dynamicSmemBytes);
     auto it = cache.find(key);
     if (it == cache.end()) {
         cfg.gridDim = dim3(kNumSM / cs * cs);
@@ -285,9 +285,11 @@ int launch_gemm_split(const SplitMaps& maps, const GemmJob* jobs, int njobs, con
     return TRIPLES_OK;
 }
 
-int launch_gemm_emu(const EmuMaps& maps, const GemmJob* jobs, int njobs, const Plan& P, const float* scales,
-                    cudaStream_t st) {
-    CU_TRY(cudaFuncSetAttribute(gemm_emu64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, EM_SMEM_BYTES));
+template <int BN>
+int launch_gemm_emu_t(const EmuMaps& maps, const GemmJob* jobs, int njobs, const Plan& P, const float* scales,
+                      cudaStream_t st) {
+    auto kern = gemm_emu64_kernel<BN>;
+    CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, em_smem_bytes(BN)));
     const int cs = P.tf_cs;
     if (njobs > EM_MAX_JOBS) return fail(TRIPLES_EINVAL, "internal: %d contraction jobs in one launch (max %d)", njobs, EM_MAX_JOBS);
     const long long items = (long long)njobs * ((P.tf_mtiles + cs - 1) / cs) * P.tf_ntiles;
@@ -297,16 +299,25 @@ int launch_gemm_emu(const EmuMaps& maps, const GemmJob* jobs, int njobs, const P
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = cs; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.blockDim = dim3(EM_THREADS);
-    cfg.dynamicSmemBytes = EM_SMEM_BYTES;
+    cfg.dynamicSmemBytes = em_smem_bytes(BN);
     cfg.stream = st;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     int max_clusters = 0;
-    if (int rc = max_pair_clusters(gemm_emu64_kernel, 1, cfg, cs, &max_clusters)) return rc;
+    if (int rc = max_pair_clusters(kern, 1 + BN / 16, cfg, cs, &max_clusters)) return rc;
     cfg.gridDim = dim3((unsigned)(std::min<long long>(items, max_clusters) * cs));
-    CU_TRY(cudaLaunchKernelEx(&cfg, gemm_emu64_kernel, maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles, P.tf_ntiles, scales));
+    CU_TRY(cudaLaunchKernelEx(&cfg, kern, maps, jobs, njobs, P.v, P.vp, P.o, P.tf_mtiles, P.tf_ntiles, scales));
     ++g_launches;
     return TRIPLES_OK;
+}
+
+int launch_gemm_emu(const EmuMaps& maps, const GemmJob* jobs, int njobs, const Plan& P, const float* scales,
+                    cudaStream_t st) {
+    switch (P.tf_bn) {
+        case 80: return launch_gemm_emu_t<80>(maps, jobs, njobs, P, scales, st);
+        case 64: return launch_gemm_emu_t<64>(maps, jobs, njobs, P, scales, st);
+        default: return launch_gemm_emu_t<48>(maps, jobs, njobs, P, scales, st);
+    }
 }
 
 int launch_gemm(const Plan& P, const Maps& maps, const Operands& op, const GemmJob* jobs, int njobs, cudaStream_t st) {

@@ -125,4 +125,5 @@ def test_parity_vs_golden_compares_the_stored_oracle_values():
     et[n, 0] *= 1 + 3e-9
     off = bench.parity_vs_golden("small", et, index, 1e-10)
     assert not off["ok"] and 2e-9 < off["max_rel_err"] < 4e-9
-    assert bench.parity_vs_golden("tiny", et, index, 1e-10) is None          # no stored file for that config name
+    assert bench.load_golden("nonexistent") is None
+    assert len(bench.load_golden("tiny")["triplets_ijk"]) == 120            # configs[0]: the C-loop golden
