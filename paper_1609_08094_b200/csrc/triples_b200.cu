@@ -370,13 +370,18 @@ struct Source {
 
 struct RunOpts { int shard = 0, nshards = 1; };
 
-int transpose_slice(const Plan& P, const double* X, double* XT, cudaStream_t st) {
-    dim3 grid((P.v + 31) / 32, (P.v + 31) / 32, P.v);     // gridDim.z <= 65535: one launch per slice
-    transpose_planes_kernel<double><<<grid, 256, 0, st>>>(X, P.v, P.vp, XT);
-    CU_TRY(cudaGetLastError());
-    ++g_launches;
+// XT = X with every (b,c) plane transposed, for `nslices` consecutive slices (v planes each); gridDim.z <= 65535
+int transpose_slices(const Plan& P, const double* X, double* XT, int nslices, cudaStream_t st) {
+    const size_t plane = (size_t)P.v * P.vp;
+    for (long long z0 = 0, nz = (long long)nslices * P.v; z0 < nz; z0 += 65535) {
+        dim3 grid((P.v + 31) / 32, (P.v + 31) / 32, (unsigned)std::min<long long>(65535, nz - z0));
+        transpose_planes_kernel<double><<<grid, 256, 0, st>>>(X + (size_t)z0 * plane, P.v, P.vp, XT + (size_t)z0 * plane);
+        CU_TRY(cudaGetLastError());
+        ++g_launches;
+    }
     return TRIPLES_OK;
 }
+int transpose_slice(const Plan& P, const double* X, double* XT, cudaStream_t st) { return transpose_slices(P, X, XT, 1, st); }
 
 // src viewed as [d][s]: the resident vvvo (ro = o, slot = r) or one FP64 slice (ro = 1) -> packed XK / XKT slots
 int pack_xk(const Plan& P, const double* src, int ro, int sp, int slot0, const Operands& op, cudaStream_t st) {
@@ -411,9 +416,7 @@ int run_prepare(const Plan& P, const Inputs& in, const Source& src, const Operan
             kern<<<(unsigned)((R + RB - 1) / RB), 256, smem, st>>>(src.vvvo, v, P.vp, o, RB, (double*)op.x);
             CU_TRY(cudaGetLastError());
             ++g_launches;
-            for (int r = 0; r < o; ++r)
-                if (int rc = transpose_slice(P, (const double*)op.x + (size_t)r * P.n_slice,
-                                             (double*)op.xt + (size_t)r * P.n_slice, st)) return rc;
+            if (int rc = transpose_slices(P, (const double*)op.x, (double*)op.xt, o, st)) return rc;
         }
         pack_ot_kernel<double><<<kNumSM * 4, 256, 0, st>>>(in.ovoo, v, o, P.op, (double*)op.ot);
         CU_TRY(cudaGetLastError());
