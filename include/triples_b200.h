@@ -108,6 +108,46 @@ int triples_energy_host(int nocc, int nvirt,
                         double* e_out, double* e_triplet_out);
 
 /*
+ * triples_energy for callers that have no device memory to give and no way to get any.
+ *
+ * Who that is: every other compute entry point takes a caller-allocated `workspace`, which presumes the caller can
+ * call cudaMalloc (or owns a pool).  Some cannot: a plug-in inside a host program (typically a quantum-chemistry
+ * package, the setting of PAPER.md L228: the canonical (T) kernel run once per small fragment) whose own memory
+ * manager has already claimed the device and hands plug-ins no allocator; code in a section that must not stall,
+ * because cudaMalloc / cudaFree synchronise the whole device and can fail late when memory is fragmented; code
+ * that runs under a rule "no allocation after start-up".  For them this entry point brings its scratch memory
+ * along: a fixed array of TRIPLES_NOALLOC_SCRATCH_BYTES that is part of the library's device image.  The call
+ * performs no cudaMalloc, cudaFree, stream / event creation or other allocating CUDA routine (profiling, which
+ * would create events, is off for its duration); the caller passes only inputs and outputs.
+ *
+ * Same arguments, results and kernels as triples_energy (Eq. (2.2.1)-(2.2.5)) minus the workspace pair.  The
+ * restricted loop is cut into narrower occupied-index windows (fewer triplets in flight) until the scratch the run
+ * needs fits the array; per-triplet arithmetic does not depend on that width.
+ *
+ *   Limit  : the array is 32 MiB, a deliberately modest figure because EVERY GPU on which this library's device
+ *            code gets loaded holds it until the process exits, used or not.  It is enough for fragment-sized
+ *            problems, roughly nocc <= 8 with nvirt <= 40 (BASELINE.json configs[0]) in all three precisions;
+ *            the need grows like 2 nocc nvirt^3 operand words.  A larger problem is refused before any GPU work
+ *            with TRIPLES_EWORKSPACE and a message naming both byte counts; such a problem needs triples_energy
+ *            and a real workspace.
+ *   Set-up : the first call on each device looks the array's device address up (cudaGetSymbolAddress, with that
+ *            device current; a failure is returned as TRIPLES_ECUDA) and keeps it.  That look-up may make the CUDA
+ *            runtime load the library's device code, which is not permitted while a stream is being captured: make
+ *            the first call on a device outside any stream capture.
+ *   Sharing: there is one array per device, shared by every call, thread and stream of the process.  A call
+ *            first zeroes the part it is going to use, so it never sees what an earlier call left behind, and
+ *            it returns after synchronising its stream.  Two calls that overlap in time on the same GPU (from
+ *            two host threads, or on two streams) write the same memory and race: results are then undefined.
+ *            Serialise them.
+ */
+#define TRIPLES_NOALLOC_SCRATCH_BYTES (32u << 20)
+int triples_energy_noalloc(int nocc, int nvirt,
+                           const double* eps_o, const double* eps_v, const double* t1, const double* t2,
+                           const double* vvvo, const double* ovoo, const double* ovov,
+                           int precision, void* cuda_stream,
+                           double* e_out, double* e_triplet_out);
+
+/*
  * Triplet-sharded run ("each loop cycle is data independent ... trivially
  * distributed", L121, L206): the batches (window blocks) of the restricted loop are cut into `nshards` contiguous
  * ranges of equal contraction-job count (triples_plan_shards); this call computes range `shard` only.

@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     triples_cache_slots,
     triples_energy,
     triples_energy_host,
+    triples_energy_noalloc,
     triples_energy_ri,
     triples_energy_sharded,
     triples_energy_streamed,

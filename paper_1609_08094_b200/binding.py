@@ -58,6 +58,8 @@ def lib() -> ctypes.CDLL:
             f = getattr(L, name)
             f.argtypes = [ctypes.c_int, ctypes.c_int] + [vp] * 7 + [ctypes.c_int, vp, ctypes.c_size_t, vp, dp, vp]
             f.restype = ctypes.c_int
+        L.triples_energy_noalloc.argtypes = [ctypes.c_int, ctypes.c_int] + [vp] * 7 + [ctypes.c_int, vp, dp, vp]
+        L.triples_energy_noalloc.restype = ctypes.c_int
         L.triples_energy_sharded.argtypes = ([ctypes.c_int, ctypes.c_int] + [vp] * 7 + [ctypes.c_int] * 3 +
                                              [vp, ctypes.c_size_t, vp, dp, vp])
         L.triples_energy_sharded.restype = ctypes.c_int
@@ -260,6 +262,23 @@ def triples_energy(nocc, nvirt, eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, precisio
     e_out = (ctypes.c_double * 3)()
     _check(lib().triples_energy(nocc, nvirt, *ptrs, precision, wp, wn, _stream_ptr(stream), e_out,
                                 _e_triplet(e_triplet_out, nocc)))
+    return float(e_out[0]), float(e_out[1]), float(e_out[2])
+
+
+NOALLOC_SCRATCH_BYTES = 32 << 20   # TRIPLES_NOALLOC_SCRATCH_BYTES of include/triples_b200.h
+
+
+def triples_energy_noalloc(nocc, nvirt, eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, precision, stream=None,
+                           e_triplet_out=None):
+    """triples_energy without a workspace argument, for callers that cannot allocate device memory (a plug-in whose
+    host program owns the device's memory, code that may not stall on cudaMalloc): the scratch is a 32 MiB array
+    inside the library's device image, so only small problems (about nocc <= 8, nvirt <= 40) are accepted; larger
+    ones raise EWORKSPACE.  One array per GPU, shared by all calls: do not overlap two calls on one GPU, and make
+    the first call on a device outside stream capture.  Returns (E(T), E[4], E[5])."""
+    ptrs = [_dev_ptr(t, n, k) for t, n, k in zip((eps_o, eps_v, t1, t2, vvvo, ovoo, ovov), _NAMES, _sizes(nocc, nvirt))]
+    e_out = (ctypes.c_double * 3)()
+    _check(lib().triples_energy_noalloc(nocc, nvirt, *ptrs, precision, _stream_ptr(stream), e_out,
+                                        _e_triplet(e_triplet_out, nocc)))
     return float(e_out[0]), float(e_out[1]), float(e_out[2])
 
 

@@ -24,6 +24,13 @@
 #include "reduce.cuh"
 #include "ri_slices.cuh"
 
+// Scratch memory of triples_energy_noalloc: part of this library's device image, so a caller that cannot allocate
+// device memory still has somewhere for the repacked operands, the U buffers and the job tables to live.  One copy per
+// GPU that loads the image, held until the process exits.  In HOST code this name is only the host-side handle of
+// the symbol, never a device address: the address a kernel may use comes from cudaGetSymbolAddress
+// (noalloc_scratch below).
+static __device__ __align__(256) unsigned char g_noalloc_scratch[TRIPLES_NOALLOC_SCRATCH_BYTES];
+
 namespace {
 
 using namespace tb;
@@ -794,6 +801,26 @@ bool fit_plan(int o, int v, int prec, int mode, int naux, size_t bytes, Plan& P)
     return false;
 }
 
+// Device address of g_noalloc_scratch on the current device: looked up once per device (with that device current),
+// then served from the table.  cudaGetSymbolAddress may load the module, hence "first call outside stream capture".
+int noalloc_scratch(uint8_t** out) {
+    static std::mutex mu;
+    static std::map<int, uint8_t*> addr;
+    int dev = 0;
+    CU_TRY(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lk(mu);
+    auto it = addr.find(dev);
+    if (it == addr.end()) {
+        void* p = nullptr;
+        CU_TRY(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255))
+            return fail(TRIPLES_ECUDA, "cudaGetSymbolAddress gave %p for the static scratch array on device %d", p, dev);
+        it = addr.emplace(dev, static_cast<uint8_t*>(p)).first;
+    }
+    *out = it->second;
+    return TRIPLES_OK;
+}
+
 }  // namespace
 
 // =============================================================================================== C ABI
@@ -961,6 +988,53 @@ int triples_energy(int nocc, int nvirt, const double* eps_o, const double* eps_v
                    size_t workspace_bytes, void* cuda_stream, double* e_out, double* e_triplet_out) {
     return triples_energy_sharded(nocc, nvirt, eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, precision, 0, 1, workspace,
                                   workspace_bytes, cuda_stream, e_out, e_triplet_out);
+}
+
+// triples_energy on the library's own static scratch array (header: who needs this, the 32 MiB limit, first-call
+// set-up, sharing).  Nothing on this path allocates: no cudaMalloc / cudaFree, no stream or event creation.
+int triples_energy_noalloc(int nocc, int nvirt, const double* eps_o, const double* eps_v, const double* t1,
+                           const double* t2, const double* vvvo, const double* ovoo, const double* ovov, int precision,
+                           void* cuda_stream, double* e_out, double* e_triplet_out) {
+    // the widest window block whose workspace fits the array (a narrower window = fewer U buffers in flight)
+    Plan P, M;
+    bool valid = false, fits = false;
+    for (int win = 4; win >= 1 && !fits; --win) {
+        if (!make_plan(nocc, nvirt, precision, M, SLICES_RESIDENT, 0, 0, win)) break;
+        valid = true;
+        if (M.win == win && M.total <= (size_t)TRIPLES_NOALLOC_SCRATCH_BYTES) { P = M; fits = true; }
+    }
+    if (!valid)
+        return fail(TRIPLES_EINVAL, "invalid sizes/precision: nocc=%d nvirt=%d precision=%d (need 1<=nocc<=%d, 1<=nvirt<=%d)",
+                    nocc, nvirt, precision, kMaxOcc, kMaxVirt);
+    if (!fits)    // M is the window-1 plan here: the least this problem can do with
+        return fail(TRIPLES_EWORKSPACE,
+                    "nocc=%d nvirt=%d precision=%d needs %zu bytes of scratch; the static array of triples_energy_noalloc "
+                    "holds %zu: use triples_energy with a workspace", nocc, nvirt, precision, M.total,
+                    (size_t)TRIPLES_NOALLOC_SCRATCH_BYTES);
+    const void* ptrs[8] = {eps_o, eps_v, t1, t2, vvvo, ovoo, ovov, e_out};
+    for (int n = 0; n < 8; ++n)
+        if (!ptrs[n]) return fail(TRIPLES_EINVAL, "null pointer argument (#%d)", n);
+    if (int rc = check_device()) return rc;
+    for (int n = 0; n < 7; ++n) {
+        if (misaligned(ptrs[n])) return fail(TRIPLES_EINVAL, "input pointer #%d is not 16-byte aligned", n);
+        if (int rc = check_device_ptr(ptrs[n], "input pointer", n)) return rc;
+    }
+    if (e_triplet_out)
+        if (int rc = check_device_ptr(e_triplet_out, "e_triplet_out", 0)) return rc;
+    uint8_t* ws = nullptr;
+    if (int rc = noalloc_scratch(&ws)) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    // the array still holds the previous call's operands, U buffers and tables (possibly of another shape or
+    // precision): everything this run is going to touch starts from zero
+    CU_TRY(cudaMemsetAsync(ws, 0, P.total, st));
+    Inputs in{eps_o, eps_v, t1, t2, ovoo, ovov};
+    Source src;
+    src.vvvo = vvvo;
+    const int profiling = g_profiling;     // profiling takes events from a pool that grows with cudaEventCreate
+    g_profiling = 0;
+    const int rc = run_full(P, in, src, ws, st, RunOpts(), e_out, e_triplet_out);
+    g_profiling = profiling;
+    return rc;
 }
 
 int triples_energy_host(int nocc, int nvirt, const double* eps_o, const double* eps_v, const double* t1,
