@@ -119,18 +119,21 @@ def oracle_sample_seconds(host, trips):
 
 
 def oracle_c_loops_rate():
-    """The plain C-loop oracle (oracle/triples_oracle.c, no BLAS) on ONE triplet of configs[1] (small: a medium
-    triplet takes it close to a minute on one core; the loops over one ijk cycle are not threaded)."""
+    """The plain C-loop oracle (oracle/triples_oracle.c, no BLAS) as SURVEY 8(d) asks for it: oracle_triples_subset is
+    OpenMP-parallel over triplets, so it gets one triplet of configs[1] (small) per host core (at least 4)."""
     from oracle import oracle
     from paper_1609_08094_b200 import synth
 
     o, v, _ = synth.CONFIGS["small"]
     inp = synth.make_config("small", seed=0)
+    cores = oracle.num_threads()
+    trips = [t for t in synth.triplet_list(o) if len(set(t)) == 3][: max(cores, 4)]
     t0 = time.perf_counter()
-    oracle.energy_subset(o, v, *inp.arrays(), [(0, 1, 2)])
+    oracle.energy_subset(o, v, *inp.arrays(), trips)
     dt = time.perf_counter() - t0
-    return {"value": (12.0 * v ** 4 + 12.0 * o * v ** 3) / dt / 1e12, "unit": "TFLOP/s", "cores": 1,
-            "kind": "oracle (plain C loops, oracle_triples_subset)", "sample": f"1 triplet (0,1,2) of small (16,120), {dt:.1f} s"}
+    return {"value": len(trips) * (12.0 * v ** 4 + 12.0 * o * v ** 3) / dt / 1e12, "unit": "TFLOP/s", "cores": cores,
+            "kind": "oracle (plain C loops, OpenMP over triplets)",
+            "sample": f"{len(trips)} triplets of small (16,120), {dt:.1f} s"}
 
 
 def blas_threads():
@@ -211,6 +214,12 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+# The timed headline stays on configs[2]: --steps 20 --warmup 5 means ~47 FP64 steps (with the e2e leg); a large /
+# largest FP64 step takes 54 s / 215 s, so those configs are one-step legs of the same command (all five configs x
+# FP64 are driver-run: tiny/small by the tests, medium here, large and largest as legs).
+WHY_MEDIUM = "20+5 steps of large/largest FP64 (54 s / 215 s each) exceed the run limit: they are 1-step legs"
+
+
 def workload_name(config, precision, o, v, naux):
     return f"{config}: nocc={o} nvirt={v} naux={naux} seed=0, {precision}, full E(T) over all i<=j<=k"
 
@@ -248,32 +257,98 @@ def parity_vs_golden(config, et, triplet_index, tol):
                       "against the timed run's e_triplet_out"}
 
 
+ROOF_KEYS = ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "share_of_step", "avg_launch_ms")
+LINE_LIMIT = 2500            # bytes: the driver keeps only the last ~3 KB of stdout, and the final line must be whole
+
+
+def _short(x):
+    """Numbers to 6 significant digits, everything else unchanged (keeps the final line small)."""
+    if isinstance(x, float):
+        return float(f"{x:.6g}")
+    if isinstance(x, dict):
+        return {k: _short(val) for k, val in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_short(val) for val in x]
+    return x
+
+
+def _pick(d, keys):
+    return None if d is None else {k: d.get(k) for k in keys if k in d}
+
+
+def leg_digest(leg):
+    """[TFLOP/s, s per E(T), contraction roofline frac, reduction roofline frac, parity max rel err] of one leg."""
+    par = leg.get("parity") or {}
+    return [leg.get("value"), leg.get("s_per_ET"), (leg.get("roofline") or {}).get("frac"),
+            (leg.get("roofline_reduction") or {}).get("frac"), par.get("max_rel_err")]
+
+
+def compact_line(full):
+    """The LAST stdout line: the contract's keys as numbers and short strings only (explanations live in DESIGN.md
+    section 10 and in the detail document, which is printed leg by leg before this line and written to a file)."""
+    keep = ("metric", "value", "executed_value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+            "scaling", "vs_baseline", "dtype", "data", "gpu_launches", "detail")
+    line = {k: full[k] for k in keep if k in full}
+    line["config"] = _pick(full.get("config"), ("workload", "parallelism", "l2"))
+    line["clocks"] = _pick(full.get("clocks"), ("sm_mhz", "sm_max_mhz", "reasons"))
+    line["roofline"] = _pick(full.get("roofline"), ROOF_KEYS)
+    line["roofline_reduction"] = _pick(full.get("roofline_reduction"), ROOF_KEYS)
+    line["cpu_baseline"] = _pick(full.get("cpu_baseline"), ("value", "unit", "cores", "kind", "sample"))
+    line["e2e"] = _pick(full.get("e2e"), ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "api"))
+    line["parity"] = _pick(full.get("parity"), ("max_rel_err", "tolerance", "ok", "triplets_compared"))
+    digest = {}
+    for name in ("mixed_path", "emu64_path", "ri_direct", "streamed"):
+        if full.get(name):
+            digest[name] = leg_digest(full[name])
+    for cfg, legs in (full.get("legs") or {}).items():
+        for name, leg in legs.items():
+            if isinstance(leg, dict) and "value" in leg:
+                digest[f"{cfg}.{name}"] = leg_digest(leg)
+    if digest:
+        line["legs"] = digest
+        line["legs_columns"] = "TFLOP/s, s_per_ET, roofline.frac, roofline_reduction.frac, parity_max_rel_err"
+    line = _short(line)
+    text = json.dumps(line, separators=(",", ":"))
+    if len(text) > LINE_LIMIT:                  # never let an over-long line reach the driver: drop the digest first
+        line.pop("legs", None)
+        line.pop("legs_columns", None)
+        text = json.dumps(line, separators=(",", ":"))
+    assert len(text) <= LINE_LIMIT, f"final bench line is {len(text)} bytes (limit {LINE_LIMIT})"
+    return text
+
+
+def emit_leg(name, leg, detail_path=None):
+    """One JSON line per leg, printed as soon as the leg is measured (the final line only carries a digest)."""
+    print(json.dumps({"leg": name, **leg}), flush=True)
+
+
+def write_detail(full, path):
+    """The whole document (every leg, every note) as a file next to the run; failure to write is not an error."""
+    try:
+        os.makedirs(os.path.dirname(path) or ".", exist_ok=True)
+        with open(path, "w") as f:
+            json.dump(full, f, indent=1)
+        return path
+    except OSError:
+        return None
+
+
 def rooflines(tb, prec, prof, peaks, peak_kind, fp64_peak, traffic):
     """Contraction (tensor pipe) and fused reduction (HBM) rooflines from one profiled step."""
     gemm_tflops = prof["contraction_flops"] / (prof["contraction_ms"] * 1e-3) / 1e12
     red_gbs = prof["reduction_bytes"] / (prof["reduction_ms"] * 1e-3) / 1e9
     step_ms = prof["prepare_ms"] + prof["contraction_ms"] + prof["reduction_ms"] + prof["other_ms"] + prof["slices_ms"]
     nl = max(prof["contraction_launches"], 1)
+    # Denominators (DESIGN.md section 10 explains each): FP64 = the DMMA peak probed in this run; EMU64 = int8 dense rate
+    # (2 x sustained bf16) / 21 digit products per FP64-class product; MIXED = 0.5 x sustained bf16 (tf32-class rate).
     if prec == tb.FP64:
-        kernel = "gemm_f64_kernel"
-        peak = fp64_peak["tflops"]
-        peak_note = fp64_peak["note"]
+        kernel, peak, peak_src = "gemm_f64_kernel", fp64_peak["tflops"], "dmma probe, this run"
     elif prec == tb.EMU64:
-        kernel = "gemm_emu64_kernel"
-        peak = peaks["bf16_tflops_sustained"] * 2.0 / 21.0
-        peak_note = (f"INT8 dense tensor rate = 2 x bf16 sustained cuBLAS ({peak_kind}, MEASURED_PEAKS.json; the guide's nominal "
-                     "int8:bf16 ratio) / 21: every FP64-class product costs 21 int8 digit products (levels <= 5 of 6 x 6 "
-                     "base-256 digits). achieved = ALGORITHMIC flops; vs_native_fp64_peak = achieved / the DMMA peak measured in "
-                     "this run (> 1: faster than the native FP64 tensor pipe can go)")
+        kernel, peak, peak_src = "gemm_emu64_kernel", peaks["bf16_tflops_sustained"] * 2.0 / 21.0, f"2 x bf16 sustained ({peak_kind}) / 21"
     else:
-        kernel = "gemm_f16split_kernel"
-        peak = peaks["bf16_tflops_sustained"] * 0.5
-        peak_note = (f"FP32-class tensor rate = 0.5 x bf16 sustained cuBLAS ({peak_kind}, MEASURED_PEAKS.json; the guide's "
-                     "nominal tf32:bf16 ratio). achieved = ALGORITHMIC flops (4v^3(v+o) per executed contraction job); the "
-                     "split h*h' + h*l' + l*h' runs as three FP16 MMAs per product, i.e. 1.5x that many tf32-rate flops "
-                     "of tensor-pipe time: tensor_pipe_tf32_equiv / frac_tensor_pipe")
+        kernel, peak, peak_src = "gemm_f16split_kernel", peaks["bf16_tflops_sustained"] * 0.5, f"0.5 x bf16 sustained ({peak_kind})"
     roof = {"bound": "tensor", "kernel": kernel, "achieved": gemm_tflops, "peak": peak, "unit": "TFLOP/s",
-            "frac": gemm_tflops / peak, "traffic": None, "peak_note": peak_note,
+            "frac": gemm_tflops / peak, "traffic": None, "peak_src": peak_src,
             "share_of_step": prof["contraction_ms"] / step_ms, "launches_per_step": prof["contraction_launches"],
             "flops_per_launch": prof["contraction_flops"] / nl, "avg_launch_ms": prof["contraction_ms"] / nl}
     if prec == tb.MIXED:
@@ -285,27 +360,24 @@ def rooflines(tb, prec, prof, peaks, peak_kind, fp64_peak, traffic):
     nr = max(prof["reduction_launches"], 1)
     red = {"bound": "hbm", "kernel": "reduce_kernel<float>" if prec == tb.MIXED else "reduce_kernel<double>",
            "achieved": red_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": red_gbs / peaks["hbm_gbs"],
-           "traffic": None,
-           "peak_note": f"{peak_kind} copy bandwidth (read + write); the reduction only reads, and a pure read stream "
-                        "can run a few per cent above a copy, so a frac slightly above 1 is a denominator mismatch, "
-                        "not skipped work",
+           "traffic": None, "peak_src": f"copy bandwidth ({peak_kind})",
            "bytes_per_launch": prof["reduction_bytes"] / nr, "avg_launch_ms": prof["reduction_ms"] / nr}
     for r in (roof, red):
         t = (traffic or {}).get(r["kernel"])
         if t:
             r["traffic"] = t["dram_bytes"]
-            r["traffic_note"] = t["note"]
-        else:
-            r["traffic_note"] = "no ncu --set full capture of this kernel at this config this round (profiles/)"
     return roof, red
 
 
 def load_traffic(config):
-    path = os.path.join(ROOT, "profiles", "r02_ncu_traffic.json")
-    if not os.path.exists(path):
-        return {}
-    with open(path) as f:
-        return json.load(f).get(config, {})
+    """ncu --set full DRAM bytes per launch of the dominant kernels (profiles/rNN_ncu_traffic.json; newest round wins)."""
+    out = {}
+    for rnd in ("r02", "r03"):
+        path = os.path.join(ROOT, "profiles", f"{rnd}_ncu_traffic.json")
+        if os.path.exists(path):
+            with open(path) as f:
+                out.update(json.load(f).get(config, {}))
+    return out
 
 
 def timed_steps(fn, steps, warmup, stream, torch):
@@ -426,6 +498,9 @@ def main():
                     help="FP64 runs only: skip the extra mixed-precision measurement reported under 'mixed_path'")
     ap.add_argument("--no-variants", action="store_true", help="skip the RI-direct and streamed measurements")
     ap.add_argument("--no-legs", action="store_true", help="skip the short legs on the large / largest configs")
+    ap.add_argument("--no-largest-fp64", action="store_true", help="legs: skip the one-step native-FP64 E(T) at largest (~215 s)")
+    ap.add_argument("--detail-out", default=os.path.join(ROOT, "gpurun_out", "bench_detail.json"),
+                    help="file that receives the whole document (all legs and notes); the last stdout line is a digest")
     ap.add_argument("--sharded", action="store_true", help="--gpus N: triplet-sharded run instead of N replicas")
     ap.add_argument("--paper-leg", action="store_true",
                     help="only the paper-size (81,323) resident + out-of-core leg in --precision (minutes; not in the default line)")
@@ -495,10 +570,7 @@ def main():
 
     # ---- roofline denominators measured in this run / on this pool
     peaks, peak_kind = measured_peaks()
-    fp64_peak = {"tflops": tb.triples_probe_fp64_peak(ws, stream=stream),
-                 "note": "FP64 tensor-core (DMMA) peak measured in this run on this device with a register-resident "
-                         "mma.sync.m8n8k4.f64 loop on all SMs (triples_probe_fp64_peak, best of 3; 148 SM x 128 flop/clk "
-                         "x 1.965 GHz = 37.2)"}
+    fp64_peak = {"tflops": tb.triples_probe_fp64_peak(ws, stream=stream)}     # DMMA issue loop on all SMs, best of 3
 
     # ---- device-resident timing: W warm-up steps, then exactly K steps between CUDA events
     sharded = args.sharded and world > 1
@@ -572,6 +644,8 @@ def main():
             "E5_abs_dev_over_abs_E4": abs(Em[2] - E[2]) / abs(E[1]),
             "note": "tolerance 1e-5 on E(T); E5 is 1e-7..1e-4 of E4 with the generator's t1 ~ N(0,1e-3^2) and a sum of both "
                     "signs, so its deviation is given on the scale of E4 (tests pin E5 with t1 ~ N(0,1))"}
+        if rank == 0:
+            emit_leg("mixed_path", mixed)
 
     # ---- FP64-class results from the INT8 tensor cores: same workload, FP64 tolerance
     emu = None
@@ -581,6 +655,8 @@ def main():
         emu["rel_dev_from_fp64"] = {"E_T": abs(Ee[0] - E[0]) / abs(E[0]), "E4": abs(Ee[1] - E[1]) / abs(E[1]),
                                     "E5": abs(Ee[2] - E[2]) / abs(E[2])}
         emu["speedup_over_fp64_path"] = (sec / args.steps) / emu["s_per_ET"]
+        if rank == 0:
+            emit_leg("emu64_path", emu)
 
     # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample (rank 0, N=1 only)
     cpu = None
@@ -591,9 +667,10 @@ def main():
         parity = float(np.max(np.abs(e_gpu[:, 0] - e_or[:, 0]) / np.abs(e_or[:, 1])))
         cpu_flops = len(trips) * (12.0 * v ** 4 + 12.0 * o * v ** 3)
         cpu = {"value": cpu_flops / dt / 1e12, "unit": "TFLOP/s", "cores": blas_threads(),
-               "kind": "oracle (numpy restatement of Eq. (2.2.1)-(2.2.5), BLAS einsum)",
-               "sample": f"{len(trips)} of {T} triplets ({trips}) via oracle.energy_subset_numpy, "
-                         f"{dt:.1f} s; full E(T) extrapolated {formula_flops(o, v)/(cpu_flops/dt):.0f} s",
+               "kind": "oracle", "oracle_form": "numpy restatement of Eq. (2.2.1)-(2.2.5), BLAS einsum",
+               "sample": f"{len(trips)} of {T} triplets, oracle.energy_subset_numpy, {dt:.1f} s "
+                         f"(full E(T) would take {formula_flops(o, v)/(cpu_flops/dt):.0f} s)",
+               "sample_triplets": trips,
                "parity_max_rel_err_on_sample": parity, "parity_ok": bool(parity <= tol),
                "parity_source": "the timed run's e_triplet_out against the oracle run here",
                "c_loops": oracle_c_loops_rate()}
@@ -622,6 +699,8 @@ def main():
         del Bd, ws_ri
         d_ = dict(dev)
         streamed = streamed_leg(tb, torch, o, v, d_, prec, stream, 12, 2, sec / args.steps, E)
+        emit_leg("ri_direct", ri)
+        emit_leg("streamed", streamed)
 
     # ---- short legs on the two largest single-GPU configs (the driver times only this default command)
     legs = None
@@ -630,7 +709,8 @@ def main():
         del dargs, dev, ws, et
         host = None
         import gc
-        for cfg, precs in (("large", (tb.FP64, tb.MIXED, tb.EMU64)), ("largest", (tb.MIXED, tb.EMU64))):
+        largest_precs = (tb.MIXED, tb.EMU64) if args.no_largest_fp64 else (tb.MIXED, tb.EMU64, tb.FP64)
+        for cfg, precs in (("large", (tb.FP64, tb.MIXED, tb.EMU64)), ("largest", largest_precs)):
             gc.collect()
             torch.cuda.empty_cache()
             lo, lv, lnaux = synth.CONFIGS[cfg]
@@ -658,6 +738,7 @@ def main():
                     lws = torch.empty(max(tb.triples_workspace_bytes(lo, lv, q) for q in precs), dtype=torch.uint8,
                                       device="cuda")
             legs[cfg] = leg
+            emit_leg("legs." + cfg, leg)
             del d, largs, lws
 
     if rank == 0:
@@ -669,11 +750,7 @@ def main():
             "config": {"workload": workload_name(args.config, args.precision, o, v, naux),
                        "parallelism": (f"triplet-sharded x{world}" if sharded else f"replicas x{world}"),
                        "l2": f"inputs larger than L2 (vvvo {8*v**3*o/1e6:.0f} MB, U buffers re-written every batch)",
-                       "flop_count": "value: T*(12v^4+12ov^3), T=o(o+1)(o+2)/6 (paper's task count, Eq. 5.0.7b); "
-                                     "executed_value: flops the kernels execute (i=j=k skipped, coinciding jobs once)",
-                       "why_this_config": "medium is the largest config whose FP64 step (3.1 s) fits the driver's "
-                                          "--steps 20 --warmup 5 protocol (47 FP64 steps incl. the e2e leg); large / "
-                                          "largest are timed as short legs of the same command (legs)"},
+                       "why_this_config": WHY_MEDIUM if default_line else None},
             "E_T": E[0], "E4": E[1], "E5": E[2],
             "clocks": clocks, "gpu_launches": int(launches),
             "roofline": roofline, "roofline_reduction": roofline_reduction,
@@ -690,7 +767,11 @@ def main():
             line["streamed"] = streamed
         if legs is not None:
             line["legs"] = legs
-        print(json.dumps(line), flush=True)
+        line["detail"] = "legs: one JSON line each above this one"
+        path = write_detail(line, args.detail_out)
+        if path:
+            line["detail"] += "; whole document: " + os.path.relpath(path, ROOT)
+        print(compact_line(line), flush=True)
     if world > 1:
         import torch.distributed as dist
 

@@ -127,3 +127,34 @@ def test_parity_vs_golden_compares_the_stored_oracle_values():
     assert not off["ok"] and 2e-9 < off["max_rel_err"] < 4e-9
     assert bench.load_golden("nonexistent") is None
     assert len(bench.load_golden("tiny")["triplets_ijk"]) == 120            # configs[0]: the C-loop golden
+
+
+def test_final_bench_line_stays_small_whatever_the_legs_carry():
+    """Round 2's default command printed one 22 KB line; the driver keeps ~3 KB of stdout and recorded `parsed: null`.
+    The last line is now a digest: the contract's keys, numbers and short strings, under bench.LINE_LIMIT bytes, however
+    much the legs and notes of the full document grow (that document goes to stdout leg by leg and to a file)."""
+    with open(os.path.join(ROOT, "profiles", "r02_bench_default.json")) as f:
+        full = json.load(f)                                      # the 22 KB document itself
+    assert len(json.dumps(full)) > 20000
+    full["legs"]["largest"]["fp64"] = dict(full["legs"]["large"]["fp64"])
+    full["roofline"]["peak_note"] = "x" * 5000                    # notes of any length never reach the line
+    full["config"]["why_this_config"] = "y" * 3000
+    full["detail"] = "legs: one JSON line each above this one; whole document: gpurun_out/bench_detail.json"
+    text = bench.compact_line(full)
+    assert len(text) < bench.LINE_LIMIT <= 2500 and "\n" not in text
+    d = json.loads(text)
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "clocks", "gpu_launches", "roofline", "roofline_reduction",
+                "cpu_baseline", "e2e", "parity"):
+        assert key in d, key
+    assert d["value"] > 0 and d["config"]["workload"].startswith("medium")
+    for r in (d["roofline"], d["roofline_reduction"]):
+        assert set(r) <= set(bench.ROOF_KEYS) and r["frac"] == pytest.approx(r["achieved"] / r["peak"], rel=1e-4)
+    assert set(d["e2e"]) == {"value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "api"}
+    assert set(d["cpu_baseline"]) == {"value", "unit", "cores", "kind", "sample"}
+    assert d["legs"]["largest.fp64"][0] == pytest.approx(full["legs"]["large"]["fp64"]["value"], rel=1e-5)
+    assert len(d["legs"]["large.mixed"]) == len(d["legs_columns"].split(","))
+    # a line that would still be too long loses its digest rather than its contract keys
+    full["legs"] = {f"cfg{n}": {"fp64": full["legs"]["large"]["fp64"]} for n in range(60)}
+    d2 = json.loads(bench.compact_line(full))
+    assert "legs" not in d2 and d2["roofline"]["frac"] == d["roofline"]["frac"]
