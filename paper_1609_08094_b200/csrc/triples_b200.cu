@@ -792,7 +792,9 @@ bool fit_plan(int o, int v, int prec, int mode, int naux, size_t bytes, Plan& P)
         if (!make_plan(o, v, prec, M, mode, 0, naux, win)) return false;
         if (M.win < win) continue;                 // capped already (U budget or o): same plan as a smaller cap
         if (M.total > bytes) continue;
-        const size_t per_slot = 2 * M.n_slice * M.esz;          // before alignment: an upper estimate, walked down
+        // X and XT slot of one slice in operand words (osz: 8 FP64, 4 on both packed paths), before alignment: the
+        // start of a walk down, so it must not be an under-estimate of the slots that fit
+        const size_t per_slot = 2 * M.n_slice * M.osz;
         long long n = M.nslots + (long long)((bytes - M.total) / per_slot) + 1;
         if (n > o) n = o;
         for (; n >= M.nslots; --n)

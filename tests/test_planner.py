@@ -90,3 +90,20 @@ def test_shards_partition_the_restricted_loop(o, v, nshards):
     assert seq == sorted(seq)
     if nb >= 4 * nshards:                                 # balanced by job count (equal task weight, L198)
         assert jps.max() <= 1.5 * jps.mean() + 200
+
+
+@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED, tb.EMU64], ids=["fp64", "mixed", "emu64"])
+@pytest.mark.parametrize("o,v,mode,naux", [(32, 400, STREAMED, 0), (24, 240, RI, 720), (16, 120, STREAMED, 0), (9, 40, RI, 50)])
+def test_cache_slots_uses_the_whole_budget(o, v, mode, naux, prec):
+    """triples_cache_slots(bytes) is the LARGEST cache that fits: n slots fit, n + 1 do not (or n == nocc).  The slot
+    size is counted in operand words (4 bytes on both packed paths); counting the emulated-FP64 path's 8-byte U
+    elements instead left about half of the extra slots unused."""
+    wsb = (lambda n, w: tb.triples_workspace_bytes_streamed(o, v, prec, n, w)) if mode == STREAMED else \
+          (lambda n, w: tb.triples_workspace_bytes_ri(o, v, naux, prec, n, w))
+    lo, hi = wsb(0, 0), wsb(o, 0)
+    for frac in (0.0, 0.23, 0.5, 0.77, 1.0):
+        budget = int(lo + frac * (hi - lo))
+        n, win = tb.triples_cache_slots(o, v, naux, prec, mode, budget)
+        assert n >= 1 and win >= 1
+        assert wsb(n, win) <= budget
+        assert n == o or wsb(n + 1, win) > budget, (n, win, budget)
