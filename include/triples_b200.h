@@ -28,6 +28,9 @@
  *     `workspace` (device, caller-owned, e.g. a torch.uint8 tensor), 256-byte aligned.
  *   - Work is enqueued on `cuda_stream` (a cudaStream_t, may be NULL for the default stream);
  *     the call synchronises that stream once before writing host outputs.
+ *   - The only state the library owns -- the copy stream of streamed runs and the CUDA events of profiled /
+ *     streamed runs -- is kept per device and per host thread: one host thread may use several GPUs in turn
+ *     (cudaSetDevice before the call).  A streamed run that fails drains its copy stream before it returns.
  *   - Errors: a triples_status_t is returned, nothing aborts or throws; a message for the last
  *     non-OK status of the calling thread is available from triples_last_error().
  *     There is no CPU fallback: on a device that is not compute capability 10.x the compute
@@ -179,8 +182,12 @@ long long triples_plan_shards(int nocc, int nvirt, int precision, int nshards, i
  * on the host for the whole launch order (Belady replacement, triples_plan_slices); the copies of batch b+2 run
  * on a library-owned copy stream while batch b+1 computes.  Same kernels and the same batches as triples_energy:
  * per-triplet energies are bitwise identical to the resident run.
- *   vvvo_absmax : TRIPLES_MIXED only: the largest |(ab|ck)| if the caller knows it (it fixes the power-of-two
- *                 operand scale); <= 0: the library scans the host tensor once (one extra pass of copies).
+ *   vvvo_absmax : TRIPLES_MIXED and TRIPLES_EMU64 (ignored by TRIPLES_FP64): the largest |(ab|ck)| if the caller
+ *                 knows it (it fixes the power-of-two operand scale of the packed operands); <= 0: the library scans
+ *                 the host tensor once (one extra pass of copies).  A value ABOVE the true maximum only costs
+ *                 precision (one bit per factor of two).  A value BELOW it would overflow FP16 (mixed) or wrap the
+ *                 top base-256 digit (emulated FP64): the repack detects any element beyond the bound the value
+ *                 implies and the call returns TRIPLES_EINVAL instead of wrong energies (e_out is then invalid).
  */
 int triples_energy_streamed(int nocc, int nvirt,
                             const double* eps_o, const double* eps_v, const double* t1, const double* t2,
@@ -295,6 +302,20 @@ long long triples_plan_batches(int nocc, int nvirt, int precision, int* batch_of
  * workspace: device, at least 148*256*8 bytes.
  */
 int triples_probe_fp64_peak(void* workspace, size_t workspace_bytes, void* cuda_stream, int iters, double* tflops_out);
+
+/*
+ * tcgen05.mma peak of the current device for the two instruction kinds the packed contractions use, in Tera-operations
+ * per second (2 x multiply-adds): kind 0 = kind::f16 (FP16 x FP16 -> FP32, M = 256 over a CTA pair, N = 256, K = 16; the
+ * TRIPLES_MIXED contraction spends three of these per FP32-class product), kind 1 = kind::i8 (S8 x S8 -> S32, N = 80,
+ * K = 32; TRIPLES_EMU64 spends 21 per FP64-class product).  An issue loop on operands resident in shared memory with
+ * TMEM accumulators and no global traffic, on every co-resident CTA pair, for about `seconds` (a short run gives the
+ * burst figure, ~2 s the figure under the power cap).  *sm_mhz_out (host or NULL): the SM clock during the loop, from
+ * clock64 / globaltimer inside the kernel.  These are the roofline denominators of the two tcgen05 contraction
+ * kernels (the precision study; SURVEY 8(d) "to be measured").
+ * workspace: device, at least 148*8 bytes.
+ */
+int triples_probe_tc_peak(int kind, double seconds, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                          double* tops_out, double* sm_mhz_out);
 
 /* Number of CUDA kernels the calling thread's last compute call (triples_energy / _host / _subset / _w_block)
  * launched (repack + contraction + reduction + finalize + total). */

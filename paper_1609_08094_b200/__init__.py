@@ -23,6 +23,7 @@ from .binding import (  # noqa: F401
     triples_plan_shards,
     triples_plan_slices,
     triples_probe_fp64_peak,
+    triples_probe_tc_peak,
     triples_set_profiling,
     triples_triplet_count,
     triples_triplet_list,

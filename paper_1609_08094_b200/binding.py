@@ -81,6 +81,8 @@ def lib() -> ctypes.CDLL:
         L.triples_plan_slices.restype = ctypes.c_longlong
         L.triples_probe_fp64_peak.argtypes = [vp, ctypes.c_size_t, vp, ctypes.c_int, dp]
         L.triples_probe_fp64_peak.restype = ctypes.c_int
+        L.triples_probe_tc_peak.argtypes = [ctypes.c_int, ctypes.c_double, vp, ctypes.c_size_t, vp, dp, dp]
+        L.triples_probe_tc_peak.restype = ctypes.c_int
         L.triples_energy_subset.argtypes = ([ctypes.c_int, ctypes.c_int] + [vp] * 7 +
                                             [ctypes.c_int, ctypes.c_int, ip, vp, ctypes.c_size_t, vp, dp])
         L.triples_energy_subset.restype = ctypes.c_int
@@ -245,6 +247,15 @@ def triples_probe_fp64_peak(workspace, stream=None, iters: int = 20000) -> float
     out = ctypes.c_double(0.0)
     _check(lib().triples_probe_fp64_peak(wp, wn, _stream_ptr(stream), iters, ctypes.byref(out)))
     return float(out.value)
+
+
+def triples_probe_tc_peak(kind: int, seconds: float, workspace, stream=None):
+    """(Tera-op/s, SM MHz during the loop) of tcgen05.mma kind::f16 (kind 0) / kind::i8 (kind 1) on the current device."""
+    wp, wn = _ws(workspace)
+    tops, mhz = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(lib().triples_probe_tc_peak(kind, float(seconds), wp, wn, _stream_ptr(stream), ctypes.byref(tops),
+                                       ctypes.byref(mhz)))
+    return float(tops.value), float(mhz.value)
 
 
 def _e_triplet(e_triplet_out, nocc, host=False):

@@ -13,7 +13,7 @@
 
 namespace tb {
 
-// Mixed-path operands (gemm_tf32.cuh) are FP32 values scaled by ONE power of two per tensor class -- 2^sg for the
+// Mixed-path operands (gemm_f16split.cuh; written pre-split into FP16 h | l rows, see below) are scaled by ONE power of two per tensor class -- 2^sg for the
 // integrals (vv|vo), (ov|oo) and 2^st for t2 -- chosen so that the largest magnitude lands in [2^13, 2^14): the main
 // term of the split product then fits FP16 (11-bit significand like TF32, twice the MMA rate; 2^14 leaves a factor 4 to
 // the FP16 maximum) and every contraction term carries the same factor 2^(sg+st), removed exactly in the epilogue.
@@ -182,8 +182,14 @@ constexpr int PKX_SMEM = 32 * PKX_PITCH * 8;
 template <int MODE>
 __global__ void __launch_bounds__(256)
 pack_xk_kernel(const double* __restrict__ src, int v, int vp, int vk, int ro, int sp, int slot0,
-               uint32_t* __restrict__ XK, uint32_t* __restrict__ XKT, const float* __restrict__ sc) {
+               uint32_t* __restrict__ XK, uint32_t* __restrict__ XKT, const float* __restrict__ sc,
+               unsigned int* __restrict__ overflow) {
     const double scale = pack_scale<MODE>(sc, 0);
+    // The scale puts the class maximum in [2^13, 2^14) (FP16 split) / [2^45, 2^46) (digits).  A scaled element at or
+    // beyond that bound means the maximum the scale was derived from was too small (a caller-supplied vvvo_absmax of a
+    // streamed run): FP16 would overflow, the top digit would wrap.  Flagged here, turned into TRIPLES_EINVAL by the host.
+    const double bound = MODE == 0 ? 16384.0 : 70368744177664.0;
+    bool over = false;
     extern __shared__ double tile[];                 // [32][PKX_PITCH]
     const int d0 = blockIdx.y * 32;
     const size_t S = (size_t)v * v * ro;
@@ -206,10 +212,12 @@ pack_xk_kernel(const double* __restrict__ src, int v, int vp, int vk, int ro, in
         const size_t bc = sg / ro;
         const int b = (int)(bc / v), c = (int)(bc % v);
         const double x = tile[lane * PKX_PITCH + s];
+        over |= fabs(x * scale) >= bound;
         const size_t base = (size_t)(slot0 + r) * plane;
         pack_store<MODE>(XK + base + ((size_t)b * vp + c) * vk, blockIdx.y, x, scale, lane);
         pack_store<MODE>(XKT + base + ((size_t)c * vp + b) * vk, blockIdx.y, x, scale, lane);
     }
+    if (over) *overflow = 1u;       // every writer stores the same value
 }
 
 // blockIdx.x = q*v + x (x = b for T2K, x = c for T2KT), blockIdx.y = chunk of 64 along the contiguous source index y,

@@ -156,7 +156,14 @@ struct EventPool {
     }
     void reset() { used = 0; }
 };
-thread_local EventPool g_events;
+// One pool per device and host thread (like the copy streams): an event belongs to the device that was current when
+// it was created, and recording it on another device's stream fails with an invalid resource handle.
+thread_local std::map<int, EventPool> g_event_pools;
+EventPool& event_pool() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) dev = -1;
+    return g_event_pools[dev];
+}
 
 // ------------------------------------------------------------------------------------------ contraction launch
 // cudaFuncSetAttribute is per device and cheap: set on every launch (no process-wide "done" flag to race on).
@@ -173,6 +180,9 @@ int launch_gemm_f64(const GemmMaps& maps, const GemmJob* jobs, int njobs, const 
     ++g_launches;
     return TRIPLES_OK;
 }
+
+// word of the scales block that pack_xk_kernel sets when a scaled (vv|vo) element exceeds its class bound
+constexpr int kOverflowWord = 14;
 
 struct Operands {   // device pointers of the repacked operands (workspace) for one precision
     void *x, *xt, *ot, *t2;
@@ -396,7 +406,8 @@ int pack_xk(const Plan& P, const double* src, int ro, int sp, int slot0, const O
     CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, PKX_SMEM));
     const size_t S = (size_t)P.v * P.v * ro;
     dim3 grid((unsigned)((S + PKX_SPAN - 1) / PKX_SPAN), P.kchunks_v);
-    kern<<<grid, 256, PKX_SMEM, st>>>(src, P.v, P.vp, P.vk, ro, sp, slot0, (uint32_t*)op.x, (uint32_t*)op.xt, op.scales);
+    kern<<<grid, 256, PKX_SMEM, st>>>(src, P.v, P.vp, P.vk, ro, sp, slot0, (uint32_t*)op.x, (uint32_t*)op.xt, op.scales,
+                                      reinterpret_cast<unsigned int*>(op.scales) + kOverflowWord);
     CU_TRY(cudaGetLastError());
     ++g_launches;
     return TRIPLES_OK;
@@ -433,7 +444,7 @@ int run_prepare(const Plan& P, const Inputs& in, const Source& src, const Operan
         ++g_launches;
         return TRIPLES_OK;
     }
-    // ---- packed paths (mixed: FP16 split; emulated FP64: base-128 digits)
+    // ---- packed paths (mixed: FP16 split; emulated FP64: base-256 digits)
     const bool emu = P.prec == TRIPLES_EMU64;
     if (P.vp != v) {
         CU_TRY(cudaMemsetAsync(op.t2k, 0, P.n_t2k * 4, st));
@@ -441,7 +452,7 @@ int run_prepare(const Plan& P, const Inputs& in, const Source& src, const Operan
     }
     {   // power-of-two scales of the two tensor classes: maxima as float bit patterns, integrals | t2
         unsigned int* mx = reinterpret_cast<unsigned int*>(op.scales + 4);
-        CU_TRY(cudaMemsetAsync(mx, 0, 32, st));     // two maxima, then (RI) two factor norms at scales + 8
+        CU_TRY(cudaMemsetAsync(mx, 0, 48, st));     // two maxima, (RI) two factor norms at scales + 8, overflow flag
         const size_t nv3 = (size_t)v * v * v;
         if (src.mode == SLICES_RESIDENT) {
             absmax_kernel<<<kNumSM * 8, 256, 0, st>>>(src.vvvo, nv3 * o, mx);
@@ -456,12 +467,12 @@ int run_prepare(const Plan& P, const Inputs& in, const Source& src, const Operan
                     double* stg = op.stage + (size_t)(r & 1) * nv3;
                     if (scanned[r & 1]) CU_TRY(cudaStreamWaitEvent(copy_st, scanned[r & 1], 0));
                     CU_TRY(cudaMemcpyAsync(stg, src.vovv_host + (size_t)r * nv3, nv3 * 8, cudaMemcpyHostToDevice, copy_st));
-                    if (int rc = g_events.get(&landed)) return rc;
+                    if (int rc = event_pool().get(&landed)) return rc;
                     CU_TRY(cudaEventRecord(landed, copy_st));
                     CU_TRY(cudaStreamWaitEvent(st, landed, 0));
                     absmax_kernel<<<kNumSM * 8, 256, 0, st>>>(stg, nv3, mx);
                     ++g_launches;
-                    if (int rc = g_events.get(&scanned[r & 1])) return rc;
+                    if (int rc = event_pool().get(&scanned[r & 1])) return rc;
                     CU_TRY(cudaEventRecord(scanned[r & 1], st));
                 }
             }
@@ -521,7 +532,7 @@ int run_batches(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws,
     Operands op = carve_operands(P, ws);
     const bool prof = g_profiling != 0;
     const bool streamed = P.mode == SLICES_STREAMED, ri = P.mode == SLICES_RI;
-    g_events.reset();
+    event_pool().reset();
 
     // ---- batches, shard, slice cache and job tables (plan.h)
     BatchPlan B;
@@ -538,14 +549,14 @@ int run_batches(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws,
     if (streamed) {
         if (int rc = copy_stream(&cs)) return rc;
         cudaEvent_t ev_start;       // the copy stream may not touch the workspace before earlier work on `st` is done
-        if (int rc = g_events.get(&ev_start)) return rc;
+        if (int rc = event_pool().get(&ev_start)) return rc;
         CU_TRY(cudaEventRecord(ev_start, st));
         CU_TRY(cudaStreamWaitEvent(cs, ev_start, 0));
     }
     cudaEvent_t ev_p0 = nullptr, ev_p1 = nullptr;
     if (prof) {
-        if (int rc = g_events.get(&ev_p0)) return rc;
-        if (int rc = g_events.get(&ev_p1)) return rc;
+        if (int rc = event_pool().get(&ev_p0)) return rc;
+        if (int rc = event_pool().get(&ev_p1)) return rc;
         CU_TRY(cudaEventRecord(ev_p0, st));
     }
     if (int rc = run_prepare(P, in, src, op, st, cs)) return rc;
@@ -559,7 +570,7 @@ int run_batches(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws,
     if (prof) CU_TRY(cudaEventRecord(ev_p1, st));
     cudaEvent_t ev_prepared = nullptr;
     if (streamed) {   // pad memsets / scale scan precede the first slice copy
-        if (int rc = g_events.get(&ev_prepared)) return rc;
+        if (int rc = event_pool().get(&ev_prepared)) return rc;
         CU_TRY(cudaEventRecord(ev_prepared, st));
         CU_TRY(cudaStreamWaitEvent(cs, ev_prepared, 0));
     }
@@ -630,7 +641,7 @@ int run_batches(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws,
                 CU_TRY(cudaMemcpyAsync(stage_of(b, l - B.lstart[b]), hsrc, nv3 * 8, cudaMemcpyHostToDevice, cs));
             h2d_bytes += (double)nv3 * 8;
         }
-        if (int rc = g_events.get(&ev_loaded[b])) return rc;
+        if (int rc = event_pool().get(&ev_loaded[b])) return rc;
         CU_TRY(cudaEventRecord(ev_loaded[b], cs));
         return TRIPLES_OK;
     };
@@ -647,7 +658,7 @@ int run_batches(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws,
         const int g0 = gj_begin[b], g1 = gj_begin[b + 1];
         cudaEvent_t e[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
         if (prof) {
-            for (int x = 0; x < 5; ++x) if (int rc = g_events.get(&e[x])) return rc;
+            for (int x = 0; x < 5; ++x) if (int rc = event_pool().get(&e[x])) return rc;
             CU_TRY(cudaEventRecord(e[4], st));
         }
         if (P.mode != SLICES_RESIDENT) {
@@ -677,7 +688,7 @@ int run_batches(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws,
         if (int rc = launch_gemm(P, maps, op, d_gj + g0, g1 - g0, st)) return rc;
         if (prof) CU_TRY(cudaEventRecord(e[1], st));
         if (streamed) {
-            if (int rc = g_events.get(&ev_gemm[b])) return rc;
+            if (int rc = event_pool().get(&ev_gemm[b])) return rc;
             CU_TRY(cudaEventRecord(ev_gemm[b], st));
             if (int rc = enqueue_copies(b + 2)) return rc;
         }
@@ -704,7 +715,7 @@ int run_batches(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws,
     }
     if (streamed) {   // later work on `st` (the caller's, or the next call) starts after the copy stream has drained
         cudaEvent_t ev_end;
-        if (int rc = g_events.get(&ev_end)) return rc;
+        if (int rc = event_pool().get(&ev_end)) return rc;
         CU_TRY(cudaEventRecord(ev_end, cs));
         CU_TRY(cudaStreamWaitEvent(st, ev_end, 0));
     }
@@ -760,8 +771,19 @@ int check_device_inputs(const void* const* ptrs, int nptr, const void* ws) {
 
 int dispatch_batches(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws, cudaStream_t st,
                      const std::vector<Triplet>& trip, double* e_trip, size_t rows, const RunOpts& opt = RunOpts()) {
-    if (P.prec != TRIPLES_MIXED) return run_batches<double>(P, in, src, ws, st, trip, e_trip, rows, opt);
-    return run_batches<float>(P, in, src, ws, st, trip, e_trip, rows, opt);
+    const int rc = P.prec != TRIPLES_MIXED ? run_batches<double>(P, in, src, ws, st, trip, e_trip, rows, opt)
+                                           : run_batches<float>(P, in, src, ws, st, trip, e_trip, rows, opt);
+    if (rc != TRIPLES_OK && P.mode == SLICES_STREAMED) {
+        // an error in the middle of a streamed run may leave slice copies queued on the library's copy stream: they
+        // must not keep writing into the caller's workspace after this call has returned
+        const std::string msg = g_err;
+        cudaStream_t cs = nullptr;
+        if (copy_stream(&cs) == TRIPLES_OK) cudaStreamSynchronize(cs);
+        cudaStreamSynchronize(st);
+        cudaGetLastError();
+        g_err = msg;
+    }
+    return rc;
 }
 
 // all restricted triplets -> e_trip rows, total, results to the caller
@@ -780,7 +802,18 @@ int run_full(const Plan& P, const Inputs& in, const Source& src, uint8_t* ws, cu
     if (e_triplet_out)
         CU_TRY(cudaMemcpyAsync(e_triplet_out, e_trip, (size_t)P.T * 3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
     CU_TRY(cudaMemcpyAsync(e_out, d_res, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    // a caller-supplied maximum of the streamed tensor fixes the operand scale of the packed paths unchecked: an
+    // element beyond it overflows FP16 (mixed) or wraps the top digit (emulated FP64) -- pack_xk_kernel flags it
+    unsigned int overflow = 0;
+    const bool trusted_max = src.mode == SLICES_STREAMED && src.absmax > 0.0 && P.prec != TRIPLES_FP64;
+    if (trusted_max)
+        CU_TRY(cudaMemcpyAsync(&overflow, reinterpret_cast<const unsigned int*>(ws + P.off_result + 64) + kOverflowWord,
+                               sizeof overflow, cudaMemcpyDeviceToHost, st));
     CU_TRY(cudaStreamSynchronize(st));
+    if (overflow)
+        return fail(TRIPLES_EINVAL, "vvvo_absmax = %g is smaller than the largest |(ab|ck)| of vovv_host: the packed operands "
+                    "overflowed and the energies are invalid (pass the true maximum, or <= 0 to let the library scan)",
+                    src.absmax);
     return TRIPLES_OK;
 }
 
@@ -820,6 +853,23 @@ int noalloc_scratch(uint8_t** out) {
         it = addr.emplace(dev, static_cast<uint8_t*>(p)).first;
     }
     *out = it->second;
+    return TRIPLES_OK;
+}
+
+template <int KIND>
+int run_tc_probe(int clusters, int batches, unsigned long long* out, cudaStream_t st) {
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.blockDim = dim3(TCP_THREADS);
+    cfg.gridDim = dim3((unsigned)clusters * 2);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    CU_TRY(cudaLaunchKernelEx(&cfg, tc_peak_kernel<KIND>, batches, out));
+    ++g_launches;
     return TRIPLES_OK;
 }
 
@@ -1160,7 +1210,7 @@ int triples_w_block(int nocc, int nvirt, const double* t2, const double* vvvo, c
     uint8_t* ws = static_cast<uint8_t*>(workspace);
     Operands op = carve_operands(P, ws);
     g_launches = 0;
-    g_events.reset();
+    event_pool().reset();
     Inputs in{nullptr, nullptr, nullptr, t2, ovoo, nullptr};
     Source src;
     src.vvvo = vvvo;
@@ -1192,10 +1242,10 @@ int triples_probe_fp64_peak(void* workspace, size_t workspace_bytes, void* cuda_
     if (int rc = check_device()) return rc;
     if (int rc = check_device_ptr(workspace, "workspace", 0)) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    g_events.reset();
+    event_pool().reset();
     cudaEvent_t e0, e1;
-    if (int rc = g_events.get(&e0)) return rc;
-    if (int rc = g_events.get(&e1)) return rc;
+    if (int rc = event_pool().get(&e0)) return rc;
+    if (int rc = event_pool().get(&e1)) return rc;
     double best = 0.0;
     for (int rep = 0; rep < 4; ++rep) {      // the first repetition warms the clocks up
         CU_TRY(cudaEventRecord(e0, st));
@@ -1211,6 +1261,61 @@ int triples_probe_fp64_peak(void* workspace, size_t workspace_bytes, void* cuda_
     }
     g_launches = 4;
     *tflops_out = best;
+    return TRIPLES_OK;
+}
+
+int triples_probe_tc_peak(int kind, double seconds, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                          double* tops_out, double* sm_mhz_out) {
+    if (!workspace || !tops_out || (kind != 0 && kind != 1) || !(seconds > 0.0) || seconds > 10.0)
+        return fail(TRIPLES_EINVAL, "triples_probe_tc_peak: bad arguments (kind 0 | 1, 0 < seconds <= 10)");
+    const size_t need = (size_t)kNumSM * sizeof(unsigned long long);
+    if (workspace_bytes < need) return fail(TRIPLES_EWORKSPACE, "workspace too small: %zu bytes given, %zu needed", workspace_bytes, need);
+    if (int rc = check_device()) return rc;
+    if (int rc = check_device_ptr(workspace, "workspace", 0)) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned long long* out = static_cast<unsigned long long*>(workspace);
+    // as many CTA pairs as are co-resident (what the contraction kernels get too)
+    int clusters = 0;
+    {
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.blockDim = dim3(TCP_THREADS);
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        if (kind == 0) { if (int rc = max_pair_clusters(tc_peak_kernel<0>, 6, cfg, 2, &clusters)) return rc; }
+        else { if (int rc = max_pair_clusters(tc_peak_kernel<1>, 7, cfg, 2, &clusters)) return rc; }
+    }
+    event_pool().reset();
+    cudaEvent_t e0, e1;
+    if (int rc = event_pool().get(&e0)) return rc;
+    if (int rc = event_pool().get(&e1)) return rc;
+    g_launches = 0;
+    const double ops_per_batch = (double)clusters * TCP_BATCH * 2.0 * 256.0 * (kind == 0 ? 256.0 * 16.0 : 80.0 * 32.0);
+    int batches = 2000;                       // calibration run, then one run of about `seconds`
+    double tops = 0.0;
+    for (int pass = 0; pass < 2; ++pass) {
+        CU_TRY(cudaMemsetAsync(out, 0, need, st));
+        CU_TRY(cudaEventRecord(e0, st));
+        if (int rc = kind == 0 ? run_tc_probe<0>(clusters, batches, out, st) : run_tc_probe<1>(clusters, batches, out, st)) return rc;
+        CU_TRY(cudaEventRecord(e1, st));
+        CU_TRY(cudaStreamSynchronize(st));
+        float ms = 0;
+        CU_TRY(cudaEventElapsedTime(&ms, e0, e1));
+        tops = ops_per_batch * batches / (ms * 1e-3) / 1e12;
+        if (pass == 0) {
+            const double want = seconds / (ms * 1e-3) * batches;
+            batches = (int)std::min(std::max(want, 2000.0), 1.0e9);
+        }
+    }
+    if (sm_mhz_out) {
+        unsigned long long h[2] = {0, 0};
+        CU_TRY(cudaMemcpyAsync(h, out, sizeof h, cudaMemcpyDeviceToHost, st));
+        CU_TRY(cudaStreamSynchronize(st));
+        *sm_mhz_out = h[1] ? (double)h[0] / (double)h[1] * 1e3 : 0.0;
+    }
+    *tops_out = tops;
     return TRIPLES_OK;
 }
 

@@ -20,7 +20,7 @@
 // FP32: the same map with the roles rotated, S(x,y,z) = S0(y,z,x) -- the reduction reads every block in all six
 // arrangements, so any relabelling of the arguments is conflict free as well -- which puts the 8 x-values of one
 // (y,z) into one aligned 32-byte chunk: in the mixed GEMM a thread owns one (y,z) = (b,c) row and all x = a columns
-// (gemm_tf32.cuh), so its epilogue is two 16-byte stores per tile instead of eight scattered words.
+// (gemm_f16split.cuh), so its epilogue is two 16-byte stores per tile instead of eight scattered words.
 // Both maps are linear over GF(2): u_swz(x,y,z) = u_swz(x,0,0) ^ u_swz(0,y,z).
 // Elements with an index >= v inside the last tile of an axis are never written and never read.
 #pragma once

@@ -128,6 +128,79 @@ def test_sharded_partials_add_up_to_the_full_run(o, v, naux, nshards, prec):
     assert np.array_equal(seen, et)
     for n in range(3):
         assert abs(tot[n] - E[n]) <= 1e-13 * abs(E[1])
+    # ... and against the oracle, not only against the library's own resident run: the union of the shards' rows
+    # and the rank-ordered total (a wrong row index after the shard selection would be common to both GPU paths)
+    (Eo, et_o) = oracle.energy_restricted(o, v, *inp.arrays(), with_triplets=True)
+    assert np.abs(seen - et_o).max() <= TOL[prec] * np.abs(et_o).max()
+    for n in range(3):
+        assert abs(tot[n] - Eo[n]) <= TOL[prec] * max(abs(Eo[n]), 1e-3 * abs(Eo[1])), (n, tot, Eo)
+
+
+@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED, tb.EMU64], ids=["fp64", "mixed", "emu64"])
+def test_sharded_small_config_against_oracle_goldens(prec):
+    """BASELINE.json configs[1] (nocc 16, nvirt 120) cut into three shards: every triplet row, collected from the
+    shard that owns it, against the stored oracle values of tests/golden/small_full.json, and the rank-ordered sum of
+    the three partials against the stored E(T), E[4], E[5] (the cycles are independent)."""
+    import json
+    import os
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "small_full.json")) as f:
+        g = json.load(f)
+    o, v, naux = synth.CONFIGS["small"]
+    assert (g["nocc"], g["nvirt"], g["naux"], g["seed"], g["complete"]) == (o, v, naux, 0, True)
+    inp = synth.make_config("small", seed=0)
+    d = dev(inp)
+    ws = ws_bytes(tb.triples_workspace_bytes(o, v, prec))
+    nshards = 3
+    _, sot, jobs = tb.triples_plan_shards(o, v, prec, nshards)
+    assert jobs.min() > 0 and jobs.max() <= 1.35 * jobs.min()
+    T = tb.triples_triplet_count(o)
+    seen = np.zeros((T, 3))
+    tot = np.zeros(3)
+    for s in range(nshards):
+        ets = torch.zeros((T, 3), dtype=torch.float64, device="cuda")
+        part = tb.triples_energy_sharded(o, v, *d, prec, s, nshards, ws, e_triplet_out=ets)
+        ets = ets.cpu().numpy()
+        assert np.all(ets[sot != s] == 0.0)
+        seen += ets
+        tot += np.array(part)
+    index = {t: n for n, t in enumerate(synth.triplet_list(o))}
+    want = np.array(g["energies"])
+    for n, t in enumerate(g["triplets_ijk"]):
+        got = seen[index[tuple(t)]]
+        if t[0] == t[1] == t[2]:
+            assert np.all(got == 0.0)
+            continue
+        s4 = abs(want[n, 1])
+        assert abs(got[0] - want[n, 0]) <= TOL[prec] * s4 and abs(got[1] - want[n, 1]) <= TOL[prec] * s4, (t, got, want[n])
+        assert abs(got[2] - want[n, 2]) <= max(TOL[prec] * s4, 100 * TOL[prec] * abs(want[n, 2])), (t, got, want[n])
+    for n in range(2):
+        assert abs(tot[n] - g["E"][n]) <= TOL[prec] * abs(g["E"][n]), (n, tot, g["E"])
+
+
+@pytest.mark.parametrize("prec", [tb.MIXED, tb.EMU64], ids=["mixed", "emu64"])
+def test_streamed_run_rejects_a_vvvo_absmax_that_is_too_small(prec):
+    """The caller's vvvo_absmax fixes the operand scale of both packed paths.  Too large only costs precision; too
+    small used to overflow FP16 (mixed) / wrap the top digit (emulated FP64) silently: now TRIPLES_EINVAL."""
+    o, v = 7, 33
+    inp = synth.make_inputs(o, v, 40, seed=3, t1_sigma=0.2)
+    # (vv|vo) and (ov|oo) share one scale (the integral class); the generator's largest (ov|oo) exceeds its largest
+    # (vv|vo) and would hide an under-stated vvvo_absmax, so the (ov|oo) block is shrunk for this test
+    inp.ovoo = np.ascontiguousarray(inp.ovoo / 64.0)
+    assert np.abs(inp.ovoo).max() < np.abs(inp.vvvo).max() / 8.0
+    E, et, d = resident(inp, prec)
+    keep, host = slice_major_host(inp)
+    nbytes = tb.triples_workspace_bytes_streamed(o, v, prec, 0, 1)
+    true_max = float(np.abs(inp.vvvo).max())
+    call = lambda m: tb.triples_energy_streamed(o, v, d[0], d[1], d[2], d[3], host, d[5], d[6], prec, ws_bytes(nbytes),
+                                                vvvo_absmax=m)
+    assert call(true_max) == E
+    Ebig = call(true_max * 5.0)                         # two to three bits of headroom wasted, nothing else
+    assert abs(Ebig[0] - E[0]) <= 8 * TOL[prec] * abs(E[0])
+    for too_small in (true_max / 2.5, true_max / 7.0):
+        with pytest.raises(tb.TriplesError) as err:
+            call(too_small)
+        assert err.value.status == 1 and "vvvo_absmax" in str(err.value)
+    assert call(0.0) == E                               # the library stays usable, and its own scan gives the same scale
 
 
 def test_host_pointer_where_a_device_pointer_is_expected_is_einval():
@@ -189,35 +262,40 @@ def _check_against_golden(g, et, o, tol):
     return n_cmp
 
 
-def test_medium_streamed_with_a_budget_below_vvvo_is_bitwise_the_resident_run():
-    """configs[2] (vvvo 2.65 GB) with a device workspace SMALLER than the vvvo tensor: window 1, six cache slots,
-    2576 batches, ~3000 slice loads.  Per-triplet energies bitwise equal to the resident run, and within 1e-10 of
-    the oracle's stored values."""
+@pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED, tb.EMU64], ids=["fp64", "mixed", "emu64"])
+def test_medium_streamed_with_a_budget_below_vvvo_is_bitwise_the_resident_run(prec):
+    """configs[2] (vvvo 2.65 GB) with a device workspace SMALLER than what it streams -- the vvvo tensor (FP64) or the
+    packed X / XT operands of all slices (mixed 2.8 GB, emulated FP64 4.2 GB): window 1, six cache slots, 2576 batches,
+    ~3000 slice loads; on the packed paths every load goes through the FP64 staging ring and is split / digitised on
+    the device.  Per-triplet energies bitwise equal to the resident run, and within the precision's tolerance of the
+    oracle's stored values."""
     o, v, naux = synth.CONFIGS["medium"]
     d = synth.make_inputs_device(o, v, naux, seed=0)
     args = [d[k] for k in ("eps_o", "eps_v", "t1", "t2", "vvvo", "ovoo", "ovov")]
     T = tb.triples_triplet_count(o)
     et = torch.zeros((T, 3), dtype=torch.float64, device="cuda")
-    ws = ws_bytes(tb.triples_workspace_bytes(o, v, tb.FP64))
-    E = tb.triples_energy(o, v, *args, tb.FP64, ws, e_triplet_out=et)
+    ws = ws_bytes(tb.triples_workspace_bytes(o, v, prec))
+    E = tb.triples_energy(o, v, *args, prec, ws, e_triplet_out=et)
     del ws
     host = torch.empty((o, v, v, v), dtype=torch.float64, pin_memory=True)
     for k in range(o):
         host[k].copy_(d["vvvo"][:, :, :, k])
     torch.cuda.synchronize()
-    nbytes = tb.triples_workspace_bytes_streamed(o, v, tb.FP64, 0, 1)
-    assert nbytes < 8 * v ** 3 * o, "the budget must be smaller than the tensor that is streamed"
-    assert tb.triples_cache_slots(o, v, 0, tb.FP64, STREAMED, nbytes) == (6, 1)
+    nbytes = tb.triples_workspace_bytes_streamed(o, v, prec, 0, 1)
+    vk = {tb.MIXED: (v + 31) // 32 * 32, tb.EMU64: (v + 63) // 64 * 96}
+    streamed_bytes = 8 * v ** 3 * o if prec == tb.FP64 else 2 * o * v * v * vk[prec] * 4
+    assert nbytes < streamed_bytes, "the budget must be smaller than the operands that are streamed"
+    assert tb.triples_cache_slots(o, v, 0, prec, STREAMED, nbytes) == (6, 1)
     ets = torch.zeros_like(et)
     Es = tb.triples_energy_streamed(o, v, d["eps_o"], d["eps_v"], d["t1"], d["t2"], host.numpy(), d["ovoo"], d["ovov"],
-                                    tb.FP64, ws_bytes(nbytes), e_triplet_out=ets)
+                                    prec, ws_bytes(nbytes), e_triplet_out=ets)
     assert Es == E and torch.equal(ets, et)
     g = _golden("medium_full")
-    assert _check_against_golden(g, ets.cpu().numpy(), o, 1e-10) >= 64
+    assert _check_against_golden(g, ets.cpu().numpy(), o, TOL[prec]) >= 64
 
 
-@pytest.mark.parametrize("name,prec", [("small", tb.FP64), ("small", tb.MIXED), ("medium", tb.FP64)],
-                         ids=["small-fp64", "small-mixed", "medium-fp64"])
+@pytest.mark.parametrize("name,prec", [("small", tb.FP64), ("small", tb.MIXED), ("small", tb.EMU64), ("medium", tb.FP64)],
+                         ids=["small-fp64", "small-mixed", "small-emu64", "medium-fp64"])
 def test_ri_direct_at_config_size_against_oracle_goldens(name, prec):
     """configs[1..2] without a vvvo tensor on the device: every stored triplet of the oracle's full goldens."""
     o, v, naux = synth.CONFIGS[name]
