@@ -339,21 +339,28 @@ def rooflines(tb, prec, prof, peaks, peak_kind, fp64_peak, traffic):
     red_gbs = prof["reduction_bytes"] / (prof["reduction_ms"] * 1e-3) / 1e9
     step_ms = prof["prepare_ms"] + prof["contraction_ms"] + prof["reduction_ms"] + prof["other_ms"] + prof["slices_ms"]
     nl = max(prof["contraction_launches"], 1)
-    # Denominators (DESIGN.md section 10 explains each): FP64 = the DMMA peak probed in this run; EMU64 = int8 dense rate
-    # (2 x sustained bf16) / 21 digit products per FP64-class product; MIXED = 0.5 x sustained bf16 (tf32-class rate).
+    # Denominators: FP64 = the DMMA peak probed in this run.  The two tcgen05 kernels: the
+    # tcgen05.mma issue-loop rate of their own instruction kind and shape probed in this run (triples_probe_tc_peak,
+    # ~2 s = under the power cap, like the kernels inside a long step) divided by the MMAs one product costs: 3 FP16
+    # MMAs per FP32-class product (mixed), 21 int8 digit products per FP64-class product (emulated FP64).  The round-2
+    # nominal-ratio figures (0.5 x / 2 x sustained cuBLAS bf16) stay beside them as peak_nominal.
+    tc = peaks.get("tc_probe")
     if prec == tb.FP64:
-        kernel, peak, peak_src = "gemm_f64_kernel", fp64_peak["tflops"], "dmma probe, this run"
+        kernel, peak, peak_src, nominal = "gemm_f64_kernel", fp64_peak["tflops"], "dmma probe, this run", None
     elif prec == tb.EMU64:
-        kernel, peak, peak_src = "gemm_emu64_kernel", peaks["bf16_tflops_sustained"] * 2.0 / 21.0, f"2 x bf16 sustained ({peak_kind}) / 21"
+        kernel, nominal = "gemm_emu64_kernel", peaks["bf16_tflops_sustained"] * 2.0 / 21.0
+        peak, peak_src = (tc["i8_sustained"] / 21.0, "tcgen05 kind::i8 probe (sustained), this run / 21") if tc else \
+                         (nominal, f"2 x bf16 sustained ({peak_kind}) / 21")
     else:
-        kernel, peak, peak_src = "gemm_f16split_kernel", peaks["bf16_tflops_sustained"] * 0.5, f"0.5 x bf16 sustained ({peak_kind})"
+        kernel, nominal = "gemm_f16split_kernel", peaks["bf16_tflops_sustained"] * 0.5
+        peak, peak_src = (tc["f16_sustained"] / 3.0, "tcgen05 kind::f16 probe (sustained), this run / 3") if tc else \
+                         (nominal, f"0.5 x bf16 sustained ({peak_kind})")
     roof = {"bound": "tensor", "kernel": kernel, "achieved": gemm_tflops, "peak": peak, "unit": "TFLOP/s",
-            "frac": gemm_tflops / peak, "traffic": None, "peak_src": peak_src,
+            "frac": gemm_tflops / peak, "traffic": None, "peak_src": peak_src, "peak_nominal": nominal,
             "share_of_step": prof["contraction_ms"] / step_ms, "launches_per_step": prof["contraction_launches"],
             "flops_per_launch": prof["contraction_flops"] / nl, "avg_launch_ms": prof["contraction_ms"] / nl}
     if prec == tb.MIXED:
-        roof["tensor_pipe_tf32_equiv"] = 1.5 * gemm_tflops
-        roof["frac_tensor_pipe"] = 1.5 * gemm_tflops / peak
+        roof["tensor_pipe_fp16"] = 3.0 * gemm_tflops          # FP16-rate work the tensor pipe executes
     if prec == tb.EMU64:
         roof["tensor_pipe_int8"] = 21.0 * gemm_tflops
         roof["vs_native_fp64_peak"] = gemm_tflops / fp64_peak["tflops"]
@@ -427,15 +434,17 @@ def dtype_name(tb, prec):
     return "f64" if prec == tb.FP64 else (MIXED_DTYPE if prec == tb.MIXED else EMU_DTYPE)
 
 
-def streamed_leg(tb, torch, o, v, d, prec, stream, nslots, win, resident_sec, E_resident):
+def streamed_leg(tb, torch, o, v, d, prec, stream, nslots, win, resident_sec, E_resident, scan=False):
     """Out-of-core run (NEXT-1): vvvo in pinned host memory (slice-major), a device cache of `nslots` slices; the
-    H2D copies of the slices are inside the timed region.  One warm-up-free timed call (the copies ARE the point)."""
+    H2D copies of the slices are inside the timed region.  One warm-up-free timed call (the copies ARE the point).
+    scan: packed precisions only -- pass vvvo_absmax = 0, i.e. what a caller pays who does not know the largest
+    |(ab|ck)| of a tensor that is not on the device: the library's own scan pass (one more H2D pass) is then timed too."""
     vv = d["vvvo"]
     host = torch.empty((o, v, v, v), dtype=torch.float64, pin_memory=True)
     for k in range(o):                                  # generator-side reshuffle to the slice-major layout
         host[k].copy_(vv[:, :, :, k])
     torch.cuda.synchronize()
-    absmax = float(vv.abs().max().item()) if prec != tb.FP64 else 0.0
+    absmax = float(vv.abs().max().item()) if (prec != tb.FP64 and not scan) else 0.0
     nbytes = tb.triples_workspace_bytes_streamed(o, v, prec, nslots, win)
     slots, w = tb.triples_cache_slots(o, v, 0, prec, 1, nbytes)
     ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
@@ -457,6 +466,8 @@ def streamed_leg(tb, torch, o, v, d, prec, stream, nslots, win, resident_sec, E_
             "device_workspace_bytes": nbytes, "vvvo_bytes": 8 * v ** 3 * o,
             "h2d_bytes_per_step": prof["h2d_bytes"] + 8 * (o + v + o * v), "slices_loaded": prof["slices_loaded"],
             "vs_resident": resident_sec / sec, "bitwise_equal_to_resident": bool(E == E_resident),
+            "vvvo_absmax": "n/a (fp64)" if prec == tb.FP64 else ("scanned by the library inside the timed call" if scan
+                                                                 else "supplied by the caller"),
             "note": "copies of batch b+2 run on a copy stream while batch b+1 computes; vs_resident = resident s / streamed s "
                     "(1.0 = transfer fully hidden)"}
 
@@ -498,6 +509,7 @@ def main():
                     help="FP64 runs only: skip the extra mixed-precision measurement reported under 'mixed_path'")
     ap.add_argument("--no-variants", action="store_true", help="skip the RI-direct and streamed measurements")
     ap.add_argument("--no-legs", action="store_true", help="skip the short legs on the large / largest configs")
+    ap.add_argument("--no-tc-probe", action="store_true", help="use the nominal-ratio tcgen05 peaks instead of probing them")
     ap.add_argument("--no-largest-fp64", action="store_true", help="legs: skip the one-step native-FP64 E(T) at largest (~215 s)")
     ap.add_argument("--detail-out", default=os.path.join(ROOT, "gpurun_out", "bench_detail.json"),
                     help="file that receives the whole document (all legs and notes); the last stdout line is a digest")
@@ -572,6 +584,23 @@ def main():
     peaks, peak_kind = measured_peaks()
     fp64_peak = {"tflops": tb.triples_probe_fp64_peak(ws, stream=stream)}     # DMMA issue loop on all SMs, best of 3
 
+    def probe_tc():
+        """tcgen05.mma issue loops: 50 ms (burst) and 2 s (under the power cap) per kind -> peaks["tc_probe"]."""
+        if args.no_tc_probe or "tc_probe" in peaks:
+            return
+        tc = {}
+        for kind, name in ((0, "f16"), (1, "i8")):
+            tc[name + "_burst"], tc[name + "_burst_mhz"] = tb.triples_probe_tc_peak(kind, 0.05, ws, stream=stream)
+            tc[name + "_sustained"], tc[name + "_sustained_mhz"] = tb.triples_probe_tc_peak(kind, 2.0, ws, stream=stream)
+        tc["unit"] = "Tera-op/s of tcgen05.mma cta_group::2 (f16: M256 N256 K16; i8: M256 N80 K32), SM MHz during the loop"
+        peaks["tc_probe"] = tc
+        if rank == 0:
+            emit_leg("tc_probe", tc)
+
+    peaks = dict(peaks)
+    if prec != tb.FP64:          # an FP64 headline does not need them: they run after its timed region (4 s at 1 kW)
+        probe_tc()
+
     # ---- device-resident timing: W warm-up steps, then exactly K steps between CUDA events
     sharded = args.sharded and world > 1
     et = torch.zeros((T, 3), dtype=torch.float64, device="cuda")
@@ -633,6 +662,8 @@ def main():
                "d2h_bytes_per_step": 24, "s_per_ET": sec_e_max / args.steps,
                "api": "triples_energy_host (C ABI, host buffers pinned)"}
         del pinned, hargs
+
+    probe_tc()
 
     # ---- the paper's other precision beside the headline one (its single/double study): same workload
     mixed = None
@@ -734,7 +765,8 @@ def main():
                 if cfg == "large" and p in (tb.FP64, tb.EMU64) and not args.no_variants:
                     del lws
                     torch.cuda.empty_cache()
-                    leg["streamed_" + key] = streamed_leg(tb, torch, lo, lv, d, p, stream, 16, 2, leg[key]["s_per_ET"], El)
+                    leg["streamed_" + key] = streamed_leg(tb, torch, lo, lv, d, p, stream, 16, 2, leg[key]["s_per_ET"], El,
+                                                          scan=(p == tb.EMU64))
                     lws = torch.empty(max(tb.triples_workspace_bytes(lo, lv, q) for q in precs), dtype=torch.uint8,
                                       device="cuda")
             legs[cfg] = leg
@@ -755,6 +787,7 @@ def main():
             "clocks": clocks, "gpu_launches": int(launches),
             "roofline": roofline, "roofline_reduction": roofline_reduction,
             "phase_ms": {k: prof[k] for k in ("prepare_ms", "contraction_ms", "reduction_ms", "other_ms")},
+            "fp64_peak_probe": fp64_peak, "tc_probe": peaks.get("tc_probe"),
             "parity": parity_golden, "e2e": e2e, "cpu_baseline": cpu,
         }
         if mixed is not None:

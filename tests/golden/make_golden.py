@@ -7,6 +7,7 @@
     python tests/golden/make_golden.py medium_t1              # configs[2] with t1 ~ N(0,1): sampled triplets, pins E[5]
     python tests/golden/make_golden.py large_sample           # configs[3]: 6 forced + 32 seeded triplets
     python tests/golden/make_golden.py largest_sample         # configs[4]: 6 forced + 32 seeded triplets
+    python tests/golden/make_golden.py paper_ala4_sample      # the paper's (nocc 81, nvirt 323) size: 6 forced + 10 seeded
         [--procs N] [--threads M]   worker processes over independent triplets x BLAS threads each
 
 The paper prints no worked numerical example of E(T) (Table 1, gives deviations from an external
@@ -46,6 +47,8 @@ JOBS = {
     "medium_t1": ("medium", 1.0, 0, 22),
     "large_sample": ("large", 1e-3, 0, 38),
     "largest_sample": ("largest", 1e-3, 0, 38),
+    # the paper's [ala]-4/cc-pVDZ size, naux = 3 nvirt, same generator: the only multi-tile ODD nvirt
+    "paper_ala4_sample": (("paper_ala4", 81, 323, 969), 1e-3, 0, 16),
 }
 
 
@@ -99,7 +102,10 @@ def _one(t):
 
 def run(name, procs, threads):
     config, t1_sigma, seed, which = JOBS[name]
-    o, v, naux = synth.CONFIGS[config]
+    if isinstance(config, tuple):                     # a size outside BASELINE.json's configs: (label, nocc, nvirt, naux)
+        config, o, v, naux = config
+    else:
+        o, v, naux = synth.CONFIGS[config]
     path = os.path.join(HERE, f"{name}.json")
     trips = synth.triplet_list(o) if which == "full" else synth.sample_triplets(o, which, seed=0)
     trips = [tuple(int(x) for x in t) for t in trips]

@@ -159,7 +159,7 @@ def test_tiny_config_full_parity_mixed(seed, t1_sigma):
 
 
 # ------------------------------------------------------------------------------------------------------------------
-# emulated-FP64 path (INT8 tensor cores, seven base-128 digits per operand) against the FP64 oracle
+# emulated-FP64 path (INT8 tensor cores, six base-256 digits per operand) against the FP64 oracle
 # at the FP64 tolerance
 # ------------------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("o,v,naux,ijk", [
@@ -305,6 +305,37 @@ def test_config_full_run_against_oracle_goldens(name, prec):
     for (a, b, c), k, x in zip(pts, ks, gotv):
         ref = float(B[:, o + a, o + b] @ B[:, o + c, k])
         assert abs(x - ref) <= 1e-12 * max(1.0, abs(ref))
+
+
+def test_paper_size_odd_nvirt_against_oracle_goldens():
+    """The paper's [ala]-4/cc-pVDZ size, nocc = 81, nvirt = 323: the only ODD nvirt that spans several
+    tiles of every kernel (323 pads to 324 columns, 3 x 120 contraction rows, 41 reduction tiles with a 3-wide tail).
+    triples_energy_subset on exactly the triplets tests/golden/paper_ala4_sample.json stores (6 forced + 10 seeded,
+    written by make_golden.py from the oracle alone), in all three precisions -- seconds, not the 8-minute full run."""
+    import gc
+    g = load_golden("paper_ala4_sample")
+    o, v, naux = g["nocc"], g["nvirt"], g["naux"]
+    assert (o, v, naux, g["seed"]) == (81, 323, 969, 0) and len(g["triplets_ijk"]) >= 16
+    _inputs_cache.clear()
+    gc.collect()
+    torch.cuda.empty_cache()
+    precs = (tb.FP64, tb.MIXED, tb.EMU64)
+    need = max(tb.triples_workspace_bytes(o, v, p) for p in precs)
+    free, _ = torch.cuda.mem_get_info()
+    if free < need + 8 * (v ** 3 * o * 1.3 + 2 * o * o * v * v):
+        pytest.skip(f"needs {need/1e9:.0f} GB of workspace next to 33 GB of inputs, {free/1e9:.0f} GB free")
+    d = synth.make_inputs_device(o, v, naux, seed=0)
+    args = [d[k] for k in NAMES]
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    trips = [tuple(t) for t in g["triplets_ijk"]]
+    index = {t: n for n, t in enumerate(trips)}
+    for prec in precs:
+        sub = tb.triples_energy_subset(o, v, *args, prec, trips, ws)
+        worst = check_triplets_against_golden(g, sub, prec, index)
+        assert worst <= TOL[prec]
+    del d, args, ws
+    gc.collect()
+    torch.cuda.empty_cache()
 
 
 @pytest.mark.parametrize("prec", [tb.FP64, tb.MIXED, tb.EMU64], ids=["fp64", "mixed", "emu64"])
@@ -492,3 +523,20 @@ def test_tiny_config_against_golden(prec):
     assert abs(E[2] - g["E"][2]) <= TOL[prec] * max(abs(g["E"][2]), 1e-3 * abs(g["E"][1]))
     got, want = et, np.array(g["triplets"])
     assert np.abs(got[:, :2] - want[:, :2]).max() <= TOL[prec] * np.abs(want[:, 1]).max()
+
+
+def test_tcgen05_peak_probes_are_sane():
+    """triples_probe_tc_peak: the issue-loop rate of the two tcgen05.mma kinds the packed contractions use -- the
+    denominators of their roofline fractions.  Nominal dense B200 rates are 2250 (fp16) and 4500 (int8) Tera-op/s; a
+    probe far below means the loop is not feeding the tensor pipe, far above means the flop count is wrong."""
+    ws = torch.empty(1 << 16, dtype=torch.uint8, device="cuda")
+    for kind, lo, hi in ((0, 900.0, 2600.0), (1, 1200.0, 5200.0)):
+        burst, mhz_b = tb.triples_probe_tc_peak(kind, 0.03, ws)
+        again, _ = tb.triples_probe_tc_peak(kind, 0.03, ws)
+        assert lo < burst < hi, (kind, burst)
+        assert 800.0 < mhz_b < 2200.0, (kind, mhz_b)
+        assert abs(again - burst) <= 0.1 * burst
+    with pytest.raises(tb.TriplesError):
+        tb.triples_probe_tc_peak(2, 0.03, ws)
+    with pytest.raises(tb.TriplesError):
+        tb.triples_probe_tc_peak(0, 0.03, torch.empty(64, dtype=torch.uint8, device="cuda"))
