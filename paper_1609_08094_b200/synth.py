@@ -51,22 +51,30 @@ class TriplesInputs:
         return (self.eps_o, self.eps_v, self.t1, self.t2, self.vvvo, self.ovoo, self.ovov)
 
 
-def draw_factors(nocc: int, nvirt: int, naux: int, seed: int = 0, t1_sigma: float = 1e-3):
-    """Random draws only (fixed order): eps_o, eps_v, symmetrised B, t1."""
+def draw_factors(nocc: int, nvirt: int, naux: int, seed: int = 0, t1_sigma: float = 1e-3, decay: float = 0.0):
+    """Random draws only (fixed order): eps_o, eps_v, symmetrised B, t1.
+
+    decay > 0 gives the integrals the structure real ones have and the flat default lacks: B[Q,p,q] is multiplied by
+    exp(-decay |p - q|) (orbital pairs far apart overlap little), so (pq|rs) spans many orders of magnitude instead of
+    one.  The draws are the same; decay = 0 leaves every stored golden value untouched."""
     rng = np.random.Generator(np.random.PCG64(seed))
     n = nocc + nvirt
     eps_o = np.sort(rng.uniform(-1.5, -0.3, size=nocc))
     eps_v = np.sort(rng.uniform(0.1, 5.0, size=nvirt))
     B = rng.normal(0.0, 0.05, size=(naux, n, n))
     B = 0.5 * (B + B.transpose(0, 2, 1))
+    if decay > 0.0:
+        idx = np.arange(n)
+        B = B * np.exp(-decay * np.abs(idx[:, None] - idx[None, :]))[None, :, :]
     t1 = rng.normal(0.0, t1_sigma, size=(nocc, nvirt))
     return eps_o, eps_v, np.ascontiguousarray(B), t1
 
 
-def make_inputs(nocc: int, nvirt: int, naux: int, seed: int = 0, t1_sigma: float = 1e-3) -> TriplesInputs:
+def make_inputs(nocc: int, nvirt: int, naux: int, seed: int = 0, t1_sigma: float = 1e-3,
+                decay: float = 0.0) -> TriplesInputs:
     """Full float64 input set on the host (numpy)."""
     o, v = nocc, nvirt
-    eps_o, eps_v, B, t1 = draw_factors(o, v, naux, seed, t1_sigma)
+    eps_o, eps_v, B, t1 = draw_factors(o, v, naux, seed, t1_sigma, decay)
     Boo = np.ascontiguousarray(B[:, :o, :o]).reshape(naux, o * o)
     Bov = np.ascontiguousarray(B[:, :o, o:]).reshape(naux, o * v)
     Bvo = np.ascontiguousarray(B[:, o:, :o]).reshape(naux, v * o)
@@ -85,9 +93,9 @@ def make_inputs(nocc: int, nvirt: int, naux: int, seed: int = 0, t1_sigma: float
                          np.ascontiguousarray(vvvo), np.ascontiguousarray(ovoo), np.ascontiguousarray(ovov))
 
 
-def make_config(name: str, seed: int = 0, t1_sigma: float = 1e-3) -> TriplesInputs:
+def make_config(name: str, seed: int = 0, t1_sigma: float = 1e-3, decay: float = 0.0) -> TriplesInputs:
     o, v, naux = CONFIGS[name]
-    return make_inputs(o, v, naux, seed, t1_sigma)
+    return make_inputs(o, v, naux, seed, t1_sigma, decay)
 
 
 def make_inputs_device(nocc: int, nvirt: int, naux: int, seed: int = 0, t1_sigma: float = 1e-3,
