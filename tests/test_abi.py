@@ -195,3 +195,22 @@ def test_plan_batches_rejects_bad_sizes(lib):
     assert lib.triples_plan_batches(3, 5, 7, None, None, None) == -1
     assert b"invalid" in lib.triples_last_error()
     assert lib.triples_plan_batches(3, 5, 0, None, None, None) > 0
+
+
+def test_decaying_generator_keeps_draws_and_symmetries():
+    """synth decay option (dynamic-range tests of the packed precisions): decay = 0 is the default generator bit for
+    bit; decay > 0 keeps the symmetries the kernels rely on and spreads the integrals over many orders of magnitude."""
+    flat = synth.make_inputs(4, 9, 12, seed=1)
+    same = synth.make_inputs(4, 9, 12, seed=1, decay=0.0)
+    for a, b in zip(flat.arrays(), same.arrays()):
+        assert np.array_equal(a, b)
+    dec = synth.make_inputs(4, 9, 12, seed=1, decay=0.6)
+    assert np.array_equal(dec.eps_o, flat.eps_o) and np.array_equal(dec.t1, flat.t1)
+    sym = lambda x, perm: np.abs(x - x.transpose(*perm)).max() <= 1e-13 * np.abs(x).max()   # up to GEMM rounding order
+    assert sym(dec.t2, (1, 0, 3, 2))                                                    # t2[i,j,a,b] = t2[j,i,b,a]
+    assert sym(dec.vvvo, (1, 0, 2, 3))                                                  # (ab|ck) = (ba|ck)
+    assert sym(dec.ovov, (2, 3, 0, 1))                                                  # (ia|jb) = (jb|ia)
+    spread = lambda x: np.abs(x).max() / np.median(np.abs(x))
+    assert spread(dec.vvvo) > 30 * spread(flat.vvvo)
+    assert all(np.all((dec.eps_o[i] + dec.eps_o[j] - dec.eps_v[:, None] - dec.eps_v[None, :]) < 0)
+               for i in range(4) for j in range(4))
