@@ -49,6 +49,12 @@
  *                FP64, everything else as TRIPLES_FP64.  Tolerance: the FP64 one.  Error model: ABSOLUTE, ~2^-46 of
  *                the class maximum per operand element (an element 2^-n below the maximum keeps 47-n bits).
  *                Every entry point takes it (streamed / RI slices are staged in FP64 and digitised on the device).
+ *                Measured on integrals that are NOT flat (synth decay option: B[Q,p,q] exp(-decay |p-q|), (vv|vo)
+ *                spanning 1e12 and more, per-triplet energies spanning 4e5 .. 6e9): E(T), E[4], E[5] stay within
+ *                6e-13 / 4e-13 / 3e-12 (EMU64) and 3e-7 (MIXED) of the oracle, and every per-triplet energy within
+ *                3e-12 (EMU64) / 2e-7 (MIXED) of the LARGEST per-triplet energy; relative to ITS OWN size a triplet
+ *                that is n orders of magnitude below the largest loses about n digits (EMU64: 1e-8 at a spread of 4e5,
+ *                1.5e-5 at 6e9) -- one power-of-two scale per tensor class, not per slice or row.
  */
 #ifndef TRIPLES_B200_H
 #define TRIPLES_B200_H
